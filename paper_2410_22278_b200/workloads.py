@@ -157,17 +157,22 @@ def _assemble(name, cell, xyz, elements, basis: _Basis, **kw) -> Workload:
 # geometry helpers
 # ----------------------------------------------------------------------------
 
-def _min_image_dist(cell: np.ndarray, a: np.ndarray, b: np.ndarray) -> float:
+_SHIFTS = np.array([[i, j, k] for i in (-1, 0, 1) for j in (-1, 0, 1) for k in (-1, 0, 1)], dtype=np.float64)
+
+
+def _min_image_dists(cell: np.ndarray, a: np.ndarray, pts: np.ndarray) -> np.ndarray:
+    """Minimum-image distances (C-21) from point a to every row of pts."""
+    if pts.shape[0] == 0:
+        return np.zeros(0)
     inv = np.linalg.inv(cell)
-    d = (a - b) @ inv
+    d = (a[None, :] - pts) @ inv
     d -= np.round(d)
-    best = float("inf")
-    for i in (-1, 0, 1):
-        for j in (-1, 0, 1):
-            for k in (-1, 0, 1):
-                v = (d + np.array([i, j, k])) @ cell
-                best = min(best, float(np.linalg.norm(v)))
-    return best
+    v = (d[:, None, :] + _SHIFTS[None, :, :]) @ cell            # (n, 27, 3)
+    return np.sqrt((v * v).sum(-1)).min(axis=1)
+
+
+def _min_image_dist(cell: np.ndarray, a: np.ndarray, b: np.ndarray) -> float:
+    return float(_min_image_dists(cell, a, b[None, :])[0])
 
 
 def _random_rotation(rng) -> np.ndarray:
@@ -201,7 +206,7 @@ def _water_box(rng, L: float, nmol: int, min_oo: float):
         for _ in range(1000):
             pos = base + rng.uniform(-1, 1, size=3) * (max_jit + 0.35 * a)
             pos = pos % L
-            if all(_min_image_dist(cell, pos, o) >= min_oo for o in O):
+            if not O or _min_image_dists(cell, pos, np.array(O)).min() >= min_oo:
                 O.append(pos)
                 break
         else:
