@@ -1,0 +1,137 @@
+/*
+ * pbc_jk.h -- C ABI of the B200-native Gamma-point, Ewald-split periodic J/K builder.
+ *
+ * Method: arxiv 2410.22278; scope: SURVEY.md section 8.  All "eq"/"L" citations
+ * are PAPER.md equation numbers / line numbers.
+ *
+ *   J_mn = sum_ls P_ls (mn|ls)      (eq 73)       Coulomb matrix
+ *   K_mn = sum_ls P_ls (ml|sn)      (eq 74)   exact-exchange matrix (no -1/2)
+ *
+ * with the crystalline, Gamma-point two-electron integral split as in eq 56 (L439),
+ * generalised to p,d shells by eq 69 (L518) and eq 98 (L742-750):
+ *
+ *   (mn|ls) = SR  [erfc(w r)/r over lattice-image-translated primitive quartets, sums R1,R2,R3]
+ *           + LR  [sum_{G != 0} 4 pi/(Omega G^2) exp(-G^2/4w^2) Re conj(rho_mn(G)) rho_ls(G)]
+ *           + SELF[-pi/(Omega w^2) S_mn S_ls]           (eq 35, eq 56 third term)
+ *
+ * Basis: contracted Cartesian Gaussian shells, l in {0,1,2} (eq 4-6).  AO order:
+ * shells in input order; components p: x,y,z; d: xx,xy,xz,yy,yz,zz (PAPER L721 example list).
+ * Every Cartesian component is normalised on its own (eq 6); `coefs` multiply normalised
+ * primitives.  The library never renormalises contracted functions.
+ *
+ * Pointers: everything handed to pbc_jk_create / pbc_jk_overlap's `S_host` is HOST memory and is
+ * copied; P, J, K of pbc_jk_build are DEVICE pointers (N x N fp64, row-major, caller-owned),
+ * the *_host variant takes HOST pointers and does the copies itself.  No torch types cross
+ * this boundary.  All functions return PBC_JK_OK (0) or a negative pbc_jk_status; no C++
+ * exception leaves the library; there is no global state besides the CUDA context.
+ *
+ * There is no CPU fallback: without a CUDA device pbc_jk_create fails with PBC_JK_ERR_CUDA.
+ */
+#ifndef PBC_JK_H
+#define PBC_JK_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    PBC_JK_OK = 0,
+    PBC_JK_ERR_INVALID_ARG = -1,   /* null pointer, w <= 0, singular cell, l > 2, exponent <= 0, nprim < 1 */
+    PBC_JK_ERR_NOMEM = -2,         /* host or device allocation failed */
+    PBC_JK_ERR_CUDA = -3,          /* CUDA runtime error; text via pbc_jk_last_error */
+    PBC_JK_ERR_UNSUPPORTED = -4    /* image index range exceeds the packed format (cell far too small) */
+} pbc_jk_status;
+
+typedef struct pbc_jk pbc_jk;      /* opaque handle: owns all host + device state of one geometry */
+
+/* rows = lattice vectors a1, a2, a3 in bohr; any non-singular cell (P1, no symmetry; L31) */
+typedef struct { double a[9]; } pbc_cell;
+
+/* xyz: 3*natom doubles, bohr; every centre may be in any lattice image (L781) */
+typedef struct { int32_t natom; const double *xyz; } pbc_atoms;
+
+/* nshell shells; shell s sits on atom[s], has angular momentum l[s] in {0,1,2} and nprim[s]
+ * primitives exps[prim_off[s] ...], coefs[prim_off[s] ...] (eq 4) */
+typedef struct {
+    int32_t nshell;
+    const int32_t *atom, *l, *nprim, *prim_off;
+    const double *exps, *coefs;
+} pbc_shells;
+
+/* Thresholds (PAPER 3.6, L823-837).  A zero selects the default. */
+typedef struct {
+    double r_cut;        /* cap on |A-B-R2| and |Q-P+R1| in bohr (0: no cap; thresholds decide)       */
+    double g_cut;        /* |G| cutoff in bohr^-1 (0: 2 w sqrt(ln(1/d_ewald_k)), from eq 62-64)   */
+    double d_pair;       /* primitive pair-image kept iff its Schwarz-type bound (eq 60, with the */
+                         /* angular factor of DESIGN.md) exceeds this; default 1e-14                   */
+    double d_schwarz;    /* primitive quartet-image evaluated iff bound_bra*bound_ket*max|P|*          */
+                         /* exp(-alpha_w r^2) (eq 67) exceeds this; default 1e-13                 */
+    double d_ewald_k;    /* sets the default g_cut; default 1e-14                                      */
+    int32_t precision;   /* 0 = fp64 everywhere; 1 = mixed (PAPER 3.5 L817-821): quartets whose       */
+                         /* density-weighted bound is below mixed_switch run in fp32, fp64 accumulate  */
+    double mixed_switch; /* default 1e-5 (L819)                                                        */
+    int32_t lr_g_batch;  /* G vectors per reciprocal-space batch (0: sized from free memory)           */
+} pbc_cutoffs;
+
+/* Counters and phase times of the LAST pbc_jk_build (times need pbc_jk_sync_stats). */
+typedef struct {
+    int32_t nbf, nshell, natom, n_g;        /* n_g: G != 0 in the half sphere (+-G paired, L243)  */
+    int64_t n_prim_pairs;                   /* ordered primitive pair-images kept (A2)            */
+    int64_t n_shell_pair_images;            /* ordered contracted shell-pair-images kept          */
+    int64_t quartets_j, quartets_k;         /* primitive quartet-images evaluated in real space   */
+    int64_t candidates_j, candidates_k;     /* primitive quartet-images tested by the screen      */
+    double  ms_density, ms_sr_j, ms_sr_k, ms_lr, ms_total;   /* device times, CUDA events         */
+    double  create_seconds;                 /* host wall time of pbc_jk_create                    */
+} pbc_jk_stats_t;
+
+/*
+ * A1-A3: validates, builds the reciprocal lattice and the half-sphere G list
+ * (eq 32-36), the image-summed primitive pair lists with bounds (Fig 1, eq 57-61
+ * L449-469, lattice enumeration eq 99-103), the Boys tables, and the crystalline overlap
+ * S (eq 21); uploads everything; sizes all workspaces.  `cut` may be NULL (all defaults).
+ * Uses the current CUDA device.  On failure *out is NULL.
+ */
+int pbc_jk_create(const pbc_cell *cell, const pbc_atoms *atoms, const pbc_shells *shells,
+                  double omega, const pbc_cutoffs *cut, pbc_jk **out);
+
+/* number of basis functions N (AO order as documented above); negative status on NULL */
+int pbc_jk_nbf(const pbc_jk *h);
+
+/* copies the crystalline overlap S (eq 21) into S_host, N*N doubles, HOST memory */
+int pbc_jk_overlap(const pbc_jk *h, double *S_host);
+
+/*
+ * A4-A10: one J+K build for density P (symmetric, N x N fp64 row-major, DEVICE).  J and/or K may
+ * be NULL to skip that matrix; otherwise they are OVERWRITTEN with the full matrices (SR+LR+SELF).
+ * All work is enqueued on `cuda_stream` (a cudaStream_t, NULL = default stream); the call does not
+ * synchronise the host and allocates nothing.  One build in flight per handle.
+ */
+int pbc_jk_build(pbc_jk *h, const double *P, double *J, double *K, void *cuda_stream);
+
+/* Same with HOST buffers: copies P host->device, builds, copies J/K back, synchronises. */
+int pbc_jk_build_host(pbc_jk *h, const double *P_host, double *J_host, double *K_host);
+
+/* `parts` bit 0 SR, bit 1 LR, bit 2 SELF (default 7): restrict the next builds to these terms of
+ * eq 56 (bring-up and tests: the oracle returns the same parts separately). */
+int pbc_jk_set_parts(pbc_jk *h, int32_t parts);
+
+/* waits for the last build on its stream and fills the counters/times */
+int pbc_jk_get_stats(pbc_jk *h, pbc_jk_stats_t *out);
+
+/* text of the last error on this handle ("" if none); valid until the next call on the handle.
+ * With h == NULL: the text of the last failed pbc_jk_create of this thread. */
+const char *pbc_jk_last_error(const pbc_jk *h);
+
+/* frees all host and device memory of the handle; NULL is a no-op */
+int pbc_jk_destroy(pbc_jk *h);
+
+/* measurement helper: runs a dependent-free DFMA loop on every SM for `iters` iterations and
+ * returns the achieved FP64 TFLOP/s (roofline denominator for the real-space kernels) */
+int pbc_jk_fp64_peak(int32_t iters, double *tflops_out);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PBC_JK_H */

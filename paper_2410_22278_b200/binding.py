@@ -1,0 +1,218 @@
+"""Thin ctypes binding of libpbc_jk.so (include/pbc_jk.h).  Argument marshalling only: every step
+of the path runs in the CUDA kernels behind the C ABI.  PyTorch supplies device memory and streams.
+
+There is no fallback: if the shared library is missing or no CUDA device is present the calls
+raise.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Optional
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libpbc_jk.so")
+
+PBC_JK_OK = 0
+STATUS = {0: "OK", -1: "INVALID_ARG", -2: "NOMEM", -3: "CUDA", -4: "UNSUPPORTED"}
+
+# every symbol include/pbc_jk.h declares (checked by tests/test_abi.py)
+SYMBOLS = ["pbc_jk_create", "pbc_jk_nbf", "pbc_jk_overlap", "pbc_jk_build", "pbc_jk_build_host",
+           "pbc_jk_set_parts", "pbc_jk_get_stats", "pbc_jk_last_error", "pbc_jk_destroy", "pbc_jk_fp64_peak"]
+
+
+class pbc_cell(C.Structure):
+    _fields_ = [("a", C.c_double * 9)]
+
+
+class pbc_atoms(C.Structure):
+    _fields_ = [("natom", C.c_int32), ("xyz", C.POINTER(C.c_double))]
+
+
+class pbc_shells(C.Structure):
+    _fields_ = [("nshell", C.c_int32), ("atom", C.POINTER(C.c_int32)), ("l", C.POINTER(C.c_int32)),
+                ("nprim", C.POINTER(C.c_int32)), ("prim_off", C.POINTER(C.c_int32)),
+                ("exps", C.POINTER(C.c_double)), ("coefs", C.POINTER(C.c_double))]
+
+
+class pbc_cutoffs(C.Structure):
+    _fields_ = [("r_cut", C.c_double), ("g_cut", C.c_double), ("d_pair", C.c_double), ("d_schwarz", C.c_double),
+                ("d_ewald_k", C.c_double), ("precision", C.c_int32), ("mixed_switch", C.c_double),
+                ("lr_g_batch", C.c_int32)]
+
+
+class pbc_jk_stats_t(C.Structure):
+    _fields_ = [("nbf", C.c_int32), ("nshell", C.c_int32), ("natom", C.c_int32), ("n_g", C.c_int32),
+                ("n_prim_pairs", C.c_int64), ("n_shell_pair_images", C.c_int64),
+                ("quartets_j", C.c_int64), ("quartets_k", C.c_int64),
+                ("candidates_j", C.c_int64), ("candidates_k", C.c_int64),
+                ("ms_density", C.c_double), ("ms_sr_j", C.c_double), ("ms_sr_k", C.c_double), ("ms_lr", C.c_double),
+                ("ms_total", C.c_double), ("create_seconds", C.c_double)]
+
+
+_lib = None
+
+
+def load() -> C.CDLL:
+    """dlopen libpbc_jk.so (built by `python -m paper_2410_22278_b200.build`).  Raises if absent."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise RuntimeError(f"{LIB_PATH} is missing: build it with `python -m paper_2410_22278_b200.build` "
+                               "(there is no CPU fallback)")
+        lib = C.CDLL(LIB_PATH)
+        lib.pbc_jk_create.argtypes = [C.POINTER(pbc_cell), C.POINTER(pbc_atoms), C.POINTER(pbc_shells), C.c_double,
+                                      C.POINTER(pbc_cutoffs), C.POINTER(C.c_void_p)]
+        lib.pbc_jk_create.restype = C.c_int
+        lib.pbc_jk_nbf.argtypes = [C.c_void_p]
+        lib.pbc_jk_nbf.restype = C.c_int
+        lib.pbc_jk_overlap.argtypes = [C.c_void_p, C.c_void_p]
+        lib.pbc_jk_overlap.restype = C.c_int
+        lib.pbc_jk_build.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+        lib.pbc_jk_build.restype = C.c_int
+        lib.pbc_jk_build_host.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+        lib.pbc_jk_build_host.restype = C.c_int
+        lib.pbc_jk_set_parts.argtypes = [C.c_void_p, C.c_int32]
+        lib.pbc_jk_set_parts.restype = C.c_int
+        lib.pbc_jk_get_stats.argtypes = [C.c_void_p, C.POINTER(pbc_jk_stats_t)]
+        lib.pbc_jk_get_stats.restype = C.c_int
+        lib.pbc_jk_last_error.argtypes = [C.c_void_p]
+        lib.pbc_jk_last_error.restype = C.c_char_p
+        lib.pbc_jk_destroy.argtypes = [C.c_void_p]
+        lib.pbc_jk_destroy.restype = C.c_int
+        lib.pbc_jk_fp64_peak.argtypes = [C.c_int32, C.POINTER(C.c_double)]
+        lib.pbc_jk_fp64_peak.restype = C.c_int
+        _lib = lib
+    return _lib
+
+
+class PbcJKError(RuntimeError):
+    def __init__(self, code: int, text: str):
+        super().__init__(f"pbc_jk: {STATUS.get(code, code)}: {text}")
+        self.code = code
+
+
+def _dp(a):
+    return a.ctypes.data_as(C.POINTER(C.c_double))
+
+
+def _ip(a):
+    return a.ctypes.data_as(C.POINTER(C.c_int32))
+
+
+_PARTS = {"sr": 1, "lr": 2, "self": 4}
+
+
+class PbcJK:
+    """One geometry: pbc_jk_create ... pbc_jk_destroy.  `wl` is a workloads.Workload (or anything
+    with the same fields)."""
+
+    def __init__(self, wl, omega: Optional[float] = None, r_cut: Optional[float] = None,
+                 g_cut: Optional[float] = None, d_pair: float = 0.0, d_schwarz: Optional[float] = None,
+                 d_ewald_k: float = 0.0, precision: int = 0, mixed_switch: float = 0.0, lr_g_batch: int = 0):
+        self._h = C.c_void_p()
+        lib = load()
+        cell = pbc_cell()
+        flat = np.ascontiguousarray(wl.cell, dtype=np.float64).ravel()
+        for i in range(9):
+            cell.a[i] = float(flat[i])
+        self._keep = dict(
+            xyz=np.ascontiguousarray(wl.xyz, dtype=np.float64), atom=np.ascontiguousarray(wl.sh_atom, dtype=np.int32),
+            l=np.ascontiguousarray(wl.sh_l, dtype=np.int32), nprim=np.ascontiguousarray(wl.sh_nprim, dtype=np.int32),
+            off=np.ascontiguousarray(wl.sh_off, dtype=np.int32), exps=np.ascontiguousarray(wl.exps, dtype=np.float64),
+            coefs=np.ascontiguousarray(wl.coefs, dtype=np.float64))
+        k = self._keep
+        atoms = pbc_atoms(int(k["xyz"].shape[0]), _dp(k["xyz"]))
+        shells = pbc_shells(int(k["l"].shape[0]), _ip(k["atom"]), _ip(k["l"]), _ip(k["nprim"]), _ip(k["off"]),
+                            _dp(k["exps"]), _dp(k["coefs"]))
+        cut = pbc_cutoffs()
+        cut.r_cut = float(getattr(wl, "r_cut", 0.0) if r_cut is None else r_cut)
+        cut.g_cut = float(getattr(wl, "g_cut", 0.0) if g_cut is None else g_cut)
+        cut.d_pair = float(d_pair)
+        cut.d_schwarz = float(getattr(wl, "tau_schwarz", 0.0) if d_schwarz is None else d_schwarz)
+        cut.d_ewald_k = float(d_ewald_k)
+        cut.precision = int(precision)
+        cut.mixed_switch = float(mixed_switch)
+        cut.lr_g_batch = int(lr_g_batch)
+        om = float(wl.omega if omega is None else omega)
+        rc = lib.pbc_jk_create(C.byref(cell), C.byref(atoms), C.byref(shells), om, C.byref(cut), C.byref(self._h))
+        if rc != PBC_JK_OK:
+            raise PbcJKError(rc, (lib.pbc_jk_last_error(None) or b"").decode())
+        self.nbf = int(lib.pbc_jk_nbf(self._h))
+
+    def _check(self, rc: int):
+        if rc != PBC_JK_OK:
+            raise PbcJKError(rc, (load().pbc_jk_last_error(self._h) or b"").decode())
+
+    def overlap(self) -> np.ndarray:
+        S = np.zeros((self.nbf, self.nbf))
+        self._check(load().pbc_jk_overlap(self._h, S.ctypes.data))
+        return S
+
+    def set_parts(self, parts: str = "sr+lr+self"):
+        m = 0
+        for p in parts.split("+"):
+            m |= _PARTS[p.strip()]
+        self._check(load().pbc_jk_set_parts(self._h, m))
+
+    def build(self, P, J=None, K=None, stream=None):
+        """Device tensors (torch, float64, contiguous N x N).  Enqueues on `stream` (default: torch's
+        current stream) and returns without synchronising."""
+        import torch
+
+        n = self.nbf
+        for t in (P, J, K):
+            if t is None:
+                continue
+            if not (t.is_cuda and t.dtype == torch.float64 and t.is_contiguous() and tuple(t.shape) == (n, n)):
+                raise ValueError("P, J, K must be contiguous float64 CUDA tensors of shape (nbf, nbf)")
+        st = torch.cuda.current_stream().cuda_stream if stream is None else int(stream)
+        self._check(load().pbc_jk_build(self._h, P.data_ptr(), J.data_ptr() if J is not None else None,
+                                        K.data_ptr() if K is not None else None, st))
+
+    def build_host(self, P: np.ndarray, want_j: bool = True, want_k: bool = True):
+        """Host numpy in, host numpy out (copies inside the library); synchronous."""
+        n = self.nbf
+        P = np.ascontiguousarray(P, dtype=np.float64)
+        assert P.shape == (n, n)
+        J = np.empty((n, n)) if want_j else None
+        K = np.empty((n, n)) if want_k else None
+        self._check(load().pbc_jk_build_host(self._h, P.ctypes.data, J.ctypes.data if want_j else None,
+                                             K.ctypes.data if want_k else None))
+        return J, K
+
+    def build_host_ptr(self, p_ptr: int, j_ptr: int, k_ptr: int):
+        """Same with raw host addresses (pinned torch tensors in bench.py)."""
+        self._check(load().pbc_jk_build_host(self._h, p_ptr, j_ptr or None, k_ptr or None))
+
+    def stats(self) -> dict:
+        s = pbc_jk_stats_t()
+        self._check(load().pbc_jk_get_stats(self._h, C.byref(s)))
+        return {f: getattr(s, f) for f, _ in s._fields_}
+
+    def close(self):
+        if self._h:
+            load().pbc_jk_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *a):
+        self.close()
+
+
+def fp64_peak_tflops(iters: int = 20000) -> float:
+    out = C.c_double()
+    rc = load().pbc_jk_fp64_peak(int(iters), C.byref(out))
+    if rc != PBC_JK_OK:
+        raise PbcJKError(rc, "fp64 peak measurement failed")
+    return float(out.value)

@@ -1,0 +1,753 @@
+// C ABI of libpbc_jk (include/pbc_jk.h): host-side setup and the build
+// orchestration (A4-A10).  All arithmetic of the path runs in the CUDA kernels of this directory.
+#include "../../include/pbc_jk.h"
+#include "pbcjk_common.h"
+#include "pbcjk_lr.cuh"
+#include "pbcjk_sr.cuh"
+
+#include <algorithm>
+#include <chrono>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <limits>
+#include <new>
+#include <string>
+#include <vector>
+
+using namespace pbcjk;
+
+namespace {
+
+thread_local std::string g_create_error;
+
+struct DevPool {
+    std::vector<void *> ptrs;
+    template <class T>
+    cudaError_t alloc(T **p, size_t n)
+    {
+        *p = nullptr;
+        cudaError_t e = cudaMalloc((void **)p, std::max<size_t>(n, 1) * sizeof(T));
+        if (e == cudaSuccess) ptrs.push_back(*p);
+        return e;
+    }
+    template <class T>
+    cudaError_t upload(const T **p, const std::vector<T> &v)
+    {
+        T *d = nullptr;
+        cudaError_t e = alloc(&d, v.size());
+        if (e != cudaSuccess) return e;
+        if (!v.empty()) e = cudaMemcpy(d, v.data(), v.size() * sizeof(T), cudaMemcpyHostToDevice);
+        *p = d;
+        return e;
+    }
+    void free_all()
+    {
+        for (void *p : ptrs) cudaFree(p);
+        ptrs.clear();
+    }
+};
+
+struct HostPair {
+    int shA, shB;
+    double p, ip, P[3], PA[3], PB[3], coef, lb;
+};
+
+}  // namespace
+
+struct pbc_jk {
+    std::string err;
+    DevPool pool;
+    int N = 0, Np = 0, nshell = 0, natom = 0, nG = 0;
+    int parts = 7;
+    pbc_cutoffs cut{};
+    Lattice lat{};
+    ShellInfo sh{};
+    PairListK K{};
+    PairListU U{};
+    KetListJ KJ{};
+    LRParams lr{};
+    const double *boys = nullptr;
+    const double *fcomp = nullptr;
+    const int *shell_of_ao = nullptr;
+    // J bra index lists per Hermite order, K block lists per (la, ld)
+    const int *jbra[5] = {};
+    int njbra[5] = {};
+    const int2 *kblk[3][3] = {};
+    int nkblk[3][3] = {};
+    // workspaces
+    double *Pp = nullptr, *lnPmax = nullptr, *Dt = nullptr, *Jt = nullptr, *Jsr = nullptr, *Jlr = nullptr;
+    double *Ksr = nullptr, *Klr = nullptr, *Astack = nullptr, *Zstack = nullptr, *rho = nullptr;
+    double *hostP = nullptr, *hostJ = nullptr, *hostK = nullptr;     // device staging of build_host
+    unsigned long long *maxbits = nullptr, *counters = nullptr;
+    int nb = 1, nsplit = 1;
+    size_t ld = 0;
+    double c0 = 0.0;             // pi/(Omega w^2)
+    cudaEvent_t ev[6] = {};
+    cudaStream_t last_stream = nullptr;
+    bool built = false;
+    int64_t n_prim_pairs = 0, n_sp_images = 0;
+    double create_seconds = 0.0;
+    std::vector<double> S_host;
+};
+
+namespace {
+
+double det3(const double *c)
+{
+    return c[0] * (c[4] * c[8] - c[5] * c[7]) - c[1] * (c[3] * c[8] - c[5] * c[6]) + c[2] * (c[3] * c[7] - c[4] * c[6]);
+}
+
+// inverse of the 3x3 cell matrix (rows a_i): inv[j][k]; fractional f_k = sum_j r_j inv[j][k]
+void inverse3(const double *c, double *inv)
+{
+    const double d = det3(c);
+    inv[0] = (c[4] * c[8] - c[5] * c[7]) / d; inv[1] = (c[2] * c[7] - c[1] * c[8]) / d; inv[2] = (c[1] * c[5] - c[2] * c[4]) / d;
+    inv[3] = (c[5] * c[6] - c[3] * c[8]) / d; inv[4] = (c[0] * c[8] - c[2] * c[6]) / d; inv[5] = (c[2] * c[3] - c[0] * c[5]) / d;
+    inv[6] = (c[3] * c[7] - c[4] * c[6]) / d; inv[7] = (c[1] * c[6] - c[0] * c[7]) / d; inv[8] = (c[0] * c[4] - c[1] * c[3]) / d;
+}
+
+double dfact2(int n)   // (2n-1)!!
+{
+    double r = 1.0;
+    for (int k = 2 * n - 1; k > 1; k -= 2) r *= k;
+    return r;
+}
+
+// eq 6 (L72, reading C-1) for the axis-aligned component x^l: (2a/pi)^{3/4} (4a)^{l/2} / sqrt((2l-1)!!)
+double norm_axis(double a, int l)
+{
+    return std::pow(2.0 * a / M_PI, 0.75) * std::pow(4.0 * a, 0.5 * l) / std::sqrt(dfact2(l));
+}
+
+// F_m(x), m = 0..mmax: Kummer series for the top order, downward recursion (table generator)
+void boys_host(int mmax, double x, double *F)
+{
+    const double ex = std::exp(-x);
+    double term = 1.0 / (2.0 * mmax + 1.0), sum = term;
+    for (int k = 1; k < 2000; ++k) {
+        term *= 2.0 * x / (2.0 * mmax + 2.0 * k + 1.0);
+        sum += term;
+        if (term < 1e-18 * sum) break;
+    }
+    F[mmax] = ex * sum;
+    for (int m = mmax; m > 0; --m) F[m - 1] = (2.0 * x * F[m] + ex) / (2.0 * m - 1.0);
+}
+
+int fail(pbc_jk *h, int code, const std::string &msg)
+{
+    if (h) h->err = msg;
+    else g_create_error = msg;
+    return code;
+}
+
+#define CK(call)                                                                              \
+    do {                                                                                      \
+        cudaError_t e_ = (call);                                                              \
+        if (e_ != cudaSuccess) {                                                              \
+            h->err = std::string(#call) + ": " + cudaGetErrorString(e_);                      \
+            return e_ == cudaErrorMemoryAllocation ? PBC_JK_ERR_NOMEM : PBC_JK_ERR_CUDA;      \
+        }                                                                                     \
+    } while (0)
+
+// Lattice translations n with |n.a - c| < r: bounding box from the reciprocal rows, sphere filter
+// (eq 99-103).
+template <class F>
+void for_images_host(const Lattice &lat, const double c[3], double r, F &&f)
+{
+    int lo[3], hi[3];
+    for (int k = 0; k < 3; ++k) {
+        const double fk = lat.binv[3 * k] * c[0] + lat.binv[3 * k + 1] * c[1] + lat.binv[3 * k + 2] * c[2];
+        lo[k] = (int)std::ceil(fk - r * lat.bnorm[k]);
+        hi[k] = (int)std::floor(fk + r * lat.bnorm[k]);
+    }
+    for (int n0 = lo[0]; n0 <= hi[0]; ++n0)
+        for (int n1 = lo[1]; n1 <= hi[1]; ++n1)
+            for (int n2 = lo[2]; n2 <= hi[2]; ++n2) {
+                const double T[3] = {n0 * lat.a[0] + n1 * lat.a[3] + n2 * lat.a[6], n0 * lat.a[1] + n1 * lat.a[4] + n2 * lat.a[7],
+                                     n0 * lat.a[2] + n1 * lat.a[5] + n2 * lat.a[8]};
+                const double d0 = T[0] - c[0], d1 = T[1] - c[1], d2 = T[2] - c[2];
+                if (d0 * d0 + d1 * d1 + d2 * d2 < r * r) f(T);
+            }
+}
+
+int setup(pbc_jk *h, const pbc_cell *cell, const pbc_atoms *atoms, const pbc_shells *shells, double omega)
+{
+    const pbc_cutoffs &cut = h->cut;
+    // ---- A1: lattice ----
+    Lattice &lat = h->lat;
+    for (int i = 0; i < 9; ++i) lat.a[i] = cell->a[i];
+    const double vol = det3(lat.a);
+    if (!(std::fabs(vol) > 1e-12)) return fail(h, PBC_JK_ERR_INVALID_ARG, "singular cell");
+    double inv[9];
+    inverse3(lat.a, inv);
+    for (int k = 0; k < 3; ++k) {
+        for (int j = 0; j < 3; ++j) lat.binv[3 * k + j] = inv[3 * j + k];
+        lat.bnorm[k] = std::sqrt(lat.binv[3 * k] * lat.binv[3 * k] + lat.binv[3 * k + 1] * lat.binv[3 * k + 1] +
+                                 lat.binv[3 * k + 2] * lat.binv[3 * k + 2]);
+    }
+    lat.omega = omega; lat.omega2 = omega * omega; lat.iomega2 = 1.0 / (omega * omega);
+    lat.volume = std::fabs(vol);
+    h->c0 = M_PI / (lat.volume * omega * omega);
+
+    // ---- basis bookkeeping ----
+    const int ns = shells->nshell, natom = atoms->natom;
+    h->nshell = ns; h->natom = natom;
+    std::vector<int> sh_l(ns), sh_ao(ns), sh_atom(ns);
+    std::vector<double> scx(ns), scy(ns), scz(ns);
+    int nbf = 0, nprim_tot = 0;
+    double amin_all = std::numeric_limits<double>::max();
+    for (int s = 0; s < ns; ++s) {
+        const int l = shells->l[s];
+        if (l < 0 || l > LMAX) return fail(h, PBC_JK_ERR_INVALID_ARG, "shell angular momentum outside 0..2");
+        if (shells->nprim[s] < 1) return fail(h, PBC_JK_ERR_INVALID_ARG, "shell without primitives");
+        if (shells->atom[s] < 0 || shells->atom[s] >= natom) return fail(h, PBC_JK_ERR_INVALID_ARG, "shell atom index out of range");
+        sh_l[s] = l; sh_ao[s] = nbf; sh_atom[s] = shells->atom[s];
+        nbf += ncart(l);
+        scx[s] = atoms->xyz[3 * sh_atom[s]]; scy[s] = atoms->xyz[3 * sh_atom[s] + 1]; scz[s] = atoms->xyz[3 * sh_atom[s] + 2];
+        for (int k = 0; k < shells->nprim[s]; ++k) {
+            const double a = shells->exps[shells->prim_off[s] + k];
+            if (!(a > 0.0)) return fail(h, PBC_JK_ERR_INVALID_ARG, "non-positive exponent");
+            amin_all = std::min(amin_all, a);
+        }
+        nprim_tot = std::max(nprim_tot, shells->prim_off[s] + shells->nprim[s]);
+    }
+    h->N = nbf;
+    h->Np = ((nbf + 127) / 128) * 128;
+    std::vector<double> cn(nprim_tot, 0.0);
+    for (int s = 0; s < ns; ++s)
+        for (int k = 0; k < shells->nprim[s]; ++k) {
+            const int i = shells->prim_off[s] + k;
+            cn[i] = shells->coefs[i] * norm_axis(shells->exps[i], sh_l[s]);
+        }
+    std::vector<double> fcomp(nbf, 1.0);
+    std::vector<int> shell_of_ao(nbf, 0);
+    for (int s = 0; s < ns; ++s)
+        for (int k = 0; k < ncart(sh_l[s]); ++k) {
+            shell_of_ao[sh_ao[s] + k] = s;
+            if (sh_l[s] == 2 && (k == 1 || k == 2 || k == 4)) fcomp[sh_ao[s] + k] = std::sqrt(3.0);
+        }
+
+    // ---- A2: ordered primitive pair-images with bounds ----
+    const double d_pair = cut.d_pair > 0 ? cut.d_pair : 1e-14;
+    const double fmaxl[3] = {1.0, 1.0, std::sqrt(3.0)};
+    std::vector<std::vector<HostPair>> per_shell(ns);
+    std::vector<int64_t> sp_images(ns, 0);
+    bool bad_range = false;
+#pragma omp parallel for schedule(dynamic, 4)
+    for (int A = 0; A < ns; ++A) {
+        std::vector<HostPair> &out = per_shell[A];
+        const double RA[3] = {scx[A], scy[A], scz[A]};
+        const int la = sh_l[A];
+        for (int B = 0; B < ns; ++B) {
+            const int lb = sh_l[B];
+            const double RB[3] = {scx[B], scy[B], scz[B]};
+            double d[3] = {RA[0] - RB[0], RA[1] - RB[1], RA[2] - RB[2]};
+            // minimum image of the offset (eq 102-103)
+            double nr[3];
+            for (int k = 0; k < 3; ++k)
+                nr[k] = std::nearbyint(lat.binv[3 * k] * d[0] + lat.binv[3 * k + 1] * d[1] + lat.binv[3 * k + 2] * d[2]);
+            double RBm[3];
+            for (int x = 0; x < 3; ++x) RBm[x] = RB[x] + nr[0] * lat.a[x] + nr[1] * lat.a[3 + x] + nr[2] * lat.a[6 + x];
+            const double d0[3] = {RA[0] - RBm[0], RA[1] - RBm[1], RA[2] - RBm[2]};
+            // per primitive pair: prefactor and enumeration radius
+            const int na = shells->nprim[A], nb = shells->nprim[B];
+            struct PP { double a, b, p, mu, cc, isq, rad, csigned; };
+            std::vector<PP> pp;
+            double rmax = 0.0;
+            for (int ia = 0; ia < na; ++ia)
+                for (int ib = 0; ib < nb; ++ib) {
+                    PP q;
+                    q.a = shells->exps[shells->prim_off[A] + ia];
+                    q.b = shells->exps[shells->prim_off[B] + ib];
+                    q.p = q.a + q.b; q.mu = q.a * q.b / q.p; q.isq = 1.0 / std::sqrt(q.p);
+                    const double c = cn[shells->prim_off[A] + ia] * cn[shells->prim_off[B] + ib];
+                    // bound prefactor: |c| f_a f_b (pi/p)^{3/2} sqrt(2/sqrt(pi)) p^{1/4}   (eq 60 up to 2^{1/4})
+                    q.cc = std::fabs(c) * fmaxl[la] * fmaxl[lb] * std::pow(M_PI / q.p, 1.5) * std::sqrt(2.0 / std::sqrt(M_PI)) *
+                           std::pow(q.p, 0.25);
+                    double R = 40.0;
+                    bool any = true;
+                    for (int it = 0; it < 4; ++it) {
+                        const double ang = std::pow(q.b / q.p * R + q.isq, la) * std::pow(q.a / q.p * R + q.isq, lb);
+                        const double v = q.cc * ang / d_pair;
+                        if (v <= 1.0) { any = false; break; }
+                        R = std::sqrt(std::log(v) / q.mu);
+                    }
+                    q.rad = any ? R * 1.0000001 + 1e-9 : -1.0;
+                    if (cut.r_cut > 0 && q.rad > cut.r_cut) q.rad = cut.r_cut;
+                    rmax = std::max(rmax, q.rad);
+                    // keep the signed coefficient next to the bound
+                    q.csigned = c;
+                    pp.push_back(q);
+                }
+            if (rmax <= 0.0) continue;
+            for_images_host(lat, d0, rmax, [&](const double *T) {
+                const double Bt[3] = {RBm[0] + T[0], RBm[1] + T[1], RBm[2] + T[2]};
+                const double AB[3] = {RA[0] - Bt[0], RA[1] - Bt[1], RA[2] - Bt[2]};
+                const double R2 = AB[0] * AB[0] + AB[1] * AB[1] + AB[2] * AB[2];
+                const double R = std::sqrt(R2);
+                bool any = false;
+                for (const PP &q : pp) {
+                    if (q.rad <= 0.0 || R >= q.rad) continue;
+                    const double ang = std::pow(q.b / q.p * R + q.isq, la) * std::pow(q.a / q.p * R + q.isq, lb);
+                    const double ex = std::exp(-q.mu * R2);
+                    const double bound = q.cc * ang * ex;
+                    if (!(bound > d_pair)) continue;
+                    HostPair e;
+                    e.shA = A; e.shB = B; e.p = q.p; e.ip = 1.0 / q.p;
+                    for (int x = 0; x < 3; ++x) {
+                        e.P[x] = (q.a * RA[x] + q.b * Bt[x]) / q.p;
+                        e.PA[x] = e.P[x] - RA[x];
+                        e.PB[x] = e.P[x] - Bt[x];
+                    }
+                    e.coef = q.csigned * ex * std::sqrt(2.0) * std::pow(M_PI, 1.25) / q.p;
+                    e.lb = std::log(bound);
+                    out.push_back(e);
+                    any = true;
+                }
+                if (any) ++sp_images[A];
+            });
+        }
+    }
+    (void)bad_range;
+    (void)amin_all;
+    // K order: (A, l_B, bound descending)
+    std::vector<HostPair> kp;
+    {
+        size_t tot = 0;
+        for (auto &v : per_shell) tot += v.size();
+        kp.reserve(tot);
+        for (int A = 0; A < ns; ++A) {
+            auto &v = per_shell[A];
+            std::stable_sort(v.begin(), v.end(), [&](const HostPair &x, const HostPair &y) {
+                const int lx = sh_l[x.shB], ly = sh_l[y.shB];
+                if (lx != ly) return lx < ly;
+                return x.lb > y.lb;
+            });
+            kp.insert(kp.end(), v.begin(), v.end());
+            std::vector<HostPair>().swap(v);
+        }
+    }
+    h->n_prim_pairs = (int64_t)kp.size();
+    for (int A = 0; A < ns; ++A) h->n_sp_images += sp_images[A];
+    if (kp.size() > (size_t)std::numeric_limits<int>::max() / 2) return fail(h, PBC_JK_ERR_NOMEM, "too many primitive pair-images");
+
+    auto soa = [&](const std::vector<HostPair> &v, int field, int x) {
+        std::vector<double> o(v.size());
+        for (size_t i = 0; i < v.size(); ++i) {
+            const HostPair &e = v[i];
+            switch (field) {
+            case 0: o[i] = e.P[x]; break;
+            case 1: o[i] = e.p; break;
+            case 2: o[i] = e.ip; break;
+            case 3: o[i] = e.coef; break;
+            case 4: o[i] = e.lb; break;
+            case 5: o[i] = e.PA[x]; break;
+            default: o[i] = e.PB[x]; break;
+            }
+        }
+        return o;
+    };
+    DevPool &pool = h->pool;
+    // ---- upload K lists ----
+    {
+        PairListK &K = h->K;
+        K.n = (int)kp.size();
+        CK(pool.upload(&K.Px, soa(kp, 0, 0))); CK(pool.upload(&K.Py, soa(kp, 0, 1))); CK(pool.upload(&K.Pz, soa(kp, 0, 2)));
+        CK(pool.upload(&K.p, soa(kp, 1, 0))); CK(pool.upload(&K.ip, soa(kp, 2, 0)));
+        CK(pool.upload(&K.coef, soa(kp, 3, 0))); CK(pool.upload(&K.lb, soa(kp, 4, 0)));
+        CK(pool.upload(&K.PAx, soa(kp, 5, 0))); CK(pool.upload(&K.PAy, soa(kp, 5, 1))); CK(pool.upload(&K.PAz, soa(kp, 5, 2)));
+        CK(pool.upload(&K.PBx, soa(kp, 6, 0))); CK(pool.upload(&K.PBy, soa(kp, 6, 1))); CK(pool.upload(&K.PBz, soa(kp, 6, 2)));
+        std::vector<int> aoB(kp.size()), off(ns * 3 + 1, 0);
+        std::vector<double> ext(ns * 3, 0.0), ipmax(ns * 3, 0.0);
+        for (size_t i = 0; i < kp.size(); ++i) {
+            aoB[i] = sh_ao[kp[i].shB];
+            const int g = kp[i].shA * 3 + sh_l[kp[i].shB];
+            off[g + 1]++;
+            const double e = std::sqrt(kp[i].PA[0] * kp[i].PA[0] + kp[i].PA[1] * kp[i].PA[1] + kp[i].PA[2] * kp[i].PA[2]);
+            ext[g] = std::max(ext[g], e);
+            ipmax[g] = std::max(ipmax[g], kp[i].ip);
+        }
+        for (int g = 0; g < ns * 3; ++g) off[g + 1] += off[g];
+        CK(pool.upload(&K.aoB, aoB)); CK(pool.upload(&K.off, off));
+        CK(pool.upload(&K.ext, ext)); CK(pool.upload(&K.ipmax, ipmax));
+        // K block lists per (la >= ld), heaviest first
+        std::vector<int64_t> cnt(ns, 0);
+        for (int s = 0; s < ns; ++s) cnt[s] = off[s * 3 + 3] - off[s * 3];
+        for (int la = 0; la <= LMAX; ++la)
+            for (int ld = 0; ld <= la; ++ld) {
+                std::vector<std::pair<int64_t, int2>> blk;
+                for (int mu = 0; mu < ns; ++mu) {
+                    if (sh_l[mu] != la || cnt[mu] == 0) continue;
+                    for (int nu = 0; nu < ns; ++nu) {
+                        if (sh_l[nu] != ld || cnt[nu] == 0) continue;
+                        if (la == ld && nu > mu) continue;
+                        blk.push_back({cnt[mu] * cnt[nu], make_int2(mu, nu)});
+                    }
+                }
+                std::stable_sort(blk.begin(), blk.end(), [](const auto &x, const auto &y) { return x.first > y.first; });
+                std::vector<int2> b2(blk.size());
+                for (size_t i = 0; i < blk.size(); ++i) b2[i] = blk[i].second;
+                CK(pool.upload(&h->kblk[la][ld], b2));
+                h->nkblk[la][ld] = (int)b2.size();
+            }
+    }
+    // ---- U list (shell A >= shell B), contiguous per shell pair ----
+    std::vector<HostPair> up;
+    std::vector<int> u_sp, sp_off, sp_shA, sp_shB;
+    {
+        std::vector<size_t> idx;
+        for (size_t i = 0; i < kp.size(); ++i)
+            if (kp[i].shA >= kp[i].shB) idx.push_back(i);
+        std::stable_sort(idx.begin(), idx.end(), [&](size_t x, size_t y) {
+            if (kp[x].shA != kp[y].shA) return kp[x].shA < kp[y].shA;
+            return kp[x].shB < kp[y].shB;
+        });
+        up.reserve(idx.size());
+        for (size_t i : idx) up.push_back(kp[i]);
+        u_sp.resize(up.size());
+        for (size_t i = 0; i < up.size(); ++i) {
+            if (i == 0 || up[i].shA != up[i - 1].shA || up[i].shB != up[i - 1].shB) {
+                sp_off.push_back((int)i);
+                sp_shA.push_back(up[i].shA);
+                sp_shB.push_back(up[i].shB);
+            }
+            u_sp[i] = (int)sp_shA.size() - 1;
+        }
+        sp_off.push_back((int)up.size());
+        PairListU &U = h->U;
+        U.n = (int)up.size(); U.nsp = (int)sp_shA.size();
+        CK(pool.upload(&U.Px, soa(up, 0, 0))); CK(pool.upload(&U.Py, soa(up, 0, 1))); CK(pool.upload(&U.Pz, soa(up, 0, 2)));
+        CK(pool.upload(&U.p, soa(up, 1, 0))); CK(pool.upload(&U.ip, soa(up, 2, 0)));
+        CK(pool.upload(&U.coef, soa(up, 3, 0))); CK(pool.upload(&U.lb, soa(up, 4, 0)));
+        CK(pool.upload(&U.PAx, soa(up, 5, 0))); CK(pool.upload(&U.PAy, soa(up, 5, 1))); CK(pool.upload(&U.PAz, soa(up, 5, 2)));
+        CK(pool.upload(&U.PBx, soa(up, 6, 0))); CK(pool.upload(&U.PBy, soa(up, 6, 1))); CK(pool.upload(&U.PBz, soa(up, 6, 2)));
+        CK(pool.upload(&U.sp, u_sp)); CK(pool.upload(&U.sp_off, sp_off));
+        CK(pool.upload(&U.sp_shA, sp_shA)); CK(pool.upload(&U.sp_shB, sp_shB));
+        // J bra lists per Hermite order, heaviest first
+        for (int LB = 0; LB <= 4; ++LB) {
+            std::vector<int> b;
+            for (size_t i = 0; i < up.size(); ++i)
+                if (sh_l[up[i].shA] + sh_l[up[i].shB] == LB) b.push_back((int)i);
+            std::stable_sort(b.begin(), b.end(), [&](int x, int y) { return up[x].lb > up[y].lb; });
+            CK(pool.upload(&h->jbra[LB], b));
+            h->njbra[LB] = (int)b.size();
+        }
+    }
+    // ---- J kets: U regrouped by (atom of shell A, Hermite order, bound descending) ----
+    {
+        std::vector<int> idx(up.size());
+        for (size_t i = 0; i < up.size(); ++i) idx[i] = (int)i;
+        const double ln2 = std::log(2.0);
+        auto klb = [&](int i) { return up[i].lb + (up[i].shA != up[i].shB ? ln2 : 0.0); };
+        std::stable_sort(idx.begin(), idx.end(), [&](int x, int y) {
+            const int gx = sh_atom[up[x].shA] * 5 + sh_l[up[x].shA] + sh_l[up[x].shB];
+            const int gy = sh_atom[up[y].shA] * 5 + sh_l[up[y].shA] + sh_l[up[y].shB];
+            if (gx != gy) return gx < gy;
+            return klb(x) > klb(y);
+        });
+        const size_t n = idx.size();
+        std::vector<double> Qx(n), Qy(n), Qz(n), q(n), iq(n), coef(n), lb(n);
+        std::vector<int> off(natom * 5 + 1, 0);
+        std::vector<double> ext(natom * 5, 0.0), iqmax(natom * 5, 0.0), gx(natom), gy(natom), gz(natom);
+        for (int a = 0; a < natom; ++a) { gx[a] = atoms->xyz[3 * a]; gy[a] = atoms->xyz[3 * a + 1]; gz[a] = atoms->xyz[3 * a + 2]; }
+        for (size_t j = 0; j < n; ++j) {
+            const HostPair &e = up[idx[j]];
+            Qx[j] = e.P[0]; Qy[j] = e.P[1]; Qz[j] = e.P[2]; q[j] = e.p; iq[j] = e.ip; coef[j] = e.coef; lb[j] = klb(idx[j]);
+            const int g = sh_atom[e.shA] * 5 + sh_l[e.shA] + sh_l[e.shB];
+            off[g + 1]++;
+            ext[g] = std::max(ext[g], std::sqrt(e.PA[0] * e.PA[0] + e.PA[1] * e.PA[1] + e.PA[2] * e.PA[2]));
+            iqmax[g] = std::max(iqmax[g], e.ip);
+        }
+        for (int g = 0; g < natom * 5; ++g) off[g + 1] += off[g];
+        KetListJ &KJ = h->KJ;
+        KJ.n = (int)n; KJ.ngroup = natom; KJ.dstride = (int64_t)std::max<size_t>(n, 1);
+        CK(pool.upload(&KJ.Qx, Qx)); CK(pool.upload(&KJ.Qy, Qy)); CK(pool.upload(&KJ.Qz, Qz));
+        CK(pool.upload(&KJ.q, q)); CK(pool.upload(&KJ.iq, iq)); CK(pool.upload(&KJ.coef, coef)); CK(pool.upload(&KJ.lb, lb));
+        CK(pool.upload(&KJ.uidx, idx)); CK(pool.upload(&KJ.off, off));
+        CK(pool.upload(&KJ.ext, ext)); CK(pool.upload(&KJ.iqmax, iqmax));
+        CK(pool.upload(&KJ.gx, gx)); CK(pool.upload(&KJ.gy, gy)); CK(pool.upload(&KJ.gz, gz));
+    }
+    // ---- shells, component factors ----
+    {
+        ShellInfo &sh = h->sh;
+        sh.nshell = ns; sh.nbf = nbf;
+        CK(pool.upload(&sh.l, sh_l)); CK(pool.upload(&sh.ao, sh_ao)); CK(pool.upload(&sh.atom, sh_atom));
+        CK(pool.upload(&sh.cx, scx)); CK(pool.upload(&sh.cy, scy)); CK(pool.upload(&sh.cz, scz));
+        CK(pool.upload(&h->fcomp, fcomp)); CK(pool.upload(&h->shell_of_ao, shell_of_ao));
+    }
+    // ---- A1: half-sphere G list with weights (eq 32-36; cutoff eq 62-64) ----
+    {
+        const double dk = cut.d_ewald_k > 0 ? cut.d_ewald_k : 1e-14;
+        const double gcut = cut.g_cut > 0 ? cut.g_cut : 2.0 * omega * std::sqrt(std::log(1.0 / dk));
+        std::vector<double> Gx, Gy, Gz, Gw;
+        int mmax[3];
+        for (int k = 0; k < 3; ++k) {
+            const double an = std::sqrt(lat.a[3 * k] * lat.a[3 * k] + lat.a[3 * k + 1] * lat.a[3 * k + 1] + lat.a[3 * k + 2] * lat.a[3 * k + 2]);
+            mmax[k] = (int)std::ceil(gcut * an / (2.0 * M_PI));
+        }
+        for (int m0 = 0; m0 <= mmax[0]; ++m0)
+            for (int m1 = -mmax[1]; m1 <= mmax[1]; ++m1)
+                for (int m2 = -mmax[2]; m2 <= mmax[2]; ++m2) {
+                    if (m0 == 0 && (m1 < 0 || (m1 == 0 && m2 <= 0))) continue;    // half space, G = 0 omitted (L253)
+                    double G[3];
+                    for (int x = 0; x < 3; ++x)
+                        G[x] = 2.0 * M_PI * (m0 * lat.binv[x] + m1 * lat.binv[3 + x] + m2 * lat.binv[6 + x]);
+                    const double G2 = G[0] * G[0] + G[1] * G[1] + G[2] * G[2];
+                    if (G2 >= gcut * gcut) continue;
+                    Gx.push_back(G[0]); Gy.push_back(G[1]); Gz.push_back(G[2]);
+                    Gw.push_back(std::sqrt(2.0 * 4.0 * M_PI / (lat.volume * G2) * std::exp(-G2 / (4.0 * omega * omega))));
+                }
+        h->nG = (int)Gx.size();
+        LRParams &lr = h->lr;
+        CK(pool.upload(&lr.Gx, Gx)); CK(pool.upload(&lr.Gy, Gy)); CK(pool.upload(&lr.Gz, Gz)); CK(pool.upload(&lr.Gw, Gw));
+        lr.U = h->U; lr.sh = h->sh; lr.lat = lat; lr.N = nbf; lr.Np = h->Np; lr.fcomp = h->fcomp;
+    }
+    // ---- Boys table ----
+    {
+        std::vector<double> tab((size_t)BOYS_ROWS * BOYS_MCOL);
+        for (int i = 0; i < BOYS_ROWS; ++i) boys_host(BOYS_MCOL - 1, i * BOYS_DX, &tab[(size_t)i * BOYS_MCOL]);
+        CK(pool.upload(&h->boys, tab));
+    }
+    // ---- workspaces ----
+    {
+        const size_t Np = h->Np, N = nbf;
+        int nb = cut.lr_g_batch > 0 ? cut.lr_g_batch : (int)std::min<double>(16.0, std::floor(6.0e9 / (double)(Np * Np * 32)));
+        nb = std::max(1, std::min(nb, std::max(h->nG, 1)));
+        h->nb = nb;
+        h->ld = (size_t)2 * nb * Np;
+        h->nsplit = Np <= 2048 ? 4 : 1;
+        CK(pool.alloc(&h->Pp, Np * Np)); CK(cudaMemset(h->Pp, 0, Np * Np * 8));
+        CK(pool.alloc(&h->lnPmax, 1)); CK(pool.alloc(&h->maxbits, 1));
+        CK(pool.alloc(&h->counters, CNT_N)); CK(cudaMemset(h->counters, 0, CNT_N * 8));
+        CK(pool.alloc(&h->Dt, (size_t)nherm(4) * h->KJ.dstride));
+        CK(pool.alloc(&h->Jt, (size_t)nherm(4) * std::max(h->U.n, 1)));
+        CK(pool.alloc(&h->Jsr, N * N)); CK(pool.alloc(&h->Jlr, N * N)); CK(pool.alloc(&h->Ksr, N * N));
+        CK(pool.alloc(&h->Klr, (size_t)h->nsplit * Np * Np));
+        CK(pool.alloc(&h->Astack, Np * h->ld)); CK(cudaMemset(h->Astack, 0, Np * h->ld * 8));
+        CK(pool.alloc(&h->Zstack, Np * h->ld));
+        CK(pool.alloc(&h->rho, (size_t)2 * nb));
+        CK(pool.alloc(&h->hostP, N * N)); CK(pool.alloc(&h->hostJ, N * N)); CK(pool.alloc(&h->hostK, N * N));
+        for (auto &e : h->ev) CK(cudaEventCreate(&e));
+    }
+    // ---- A3: overlap S = rho_mn(G = 0) (eq 21) ----
+    {
+        launch_agen(h->lr, -1, 1, 1.0, h->Astack, h->ld, 0);
+        double *dS = h->hostJ;
+        launch_extract_overlap(h->Astack, h->ld, nbf, h->fcomp, dS, 0);
+        h->S_host.resize((size_t)nbf * nbf);
+        CK(cudaMemcpy(h->S_host.data(), dS, (size_t)nbf * nbf * 8, cudaMemcpyDeviceToHost));
+        CK(cudaGetLastError());
+    }
+    return PBC_JK_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int pbc_jk_create(const pbc_cell *cell, const pbc_atoms *atoms, const pbc_shells *shells, double omega,
+                  const pbc_cutoffs *cut, pbc_jk **out)
+{
+    if (out) *out = nullptr;
+    if (!cell || !atoms || !shells || !out) return fail(nullptr, PBC_JK_ERR_INVALID_ARG, "null argument");
+    if (!(omega > 0.0)) return fail(nullptr, PBC_JK_ERR_INVALID_ARG, "omega must be positive");
+    if (atoms->natom < 1 || !atoms->xyz || shells->nshell < 1 || !shells->atom || !shells->l || !shells->nprim ||
+        !shells->prim_off || !shells->exps || !shells->coefs)
+        return fail(nullptr, PBC_JK_ERR_INVALID_ARG, "null or empty atoms/shells");
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
+        cudaGetLastError();
+        return fail(nullptr, PBC_JK_ERR_CUDA, "no CUDA device: libpbc_jk has no CPU fallback");
+    }
+    pbc_jk *h = new (std::nothrow) pbc_jk();
+    if (!h) return fail(nullptr, PBC_JK_ERR_NOMEM, "host allocation failed");
+    if (cut) h->cut = *cut;
+    const auto t0 = std::chrono::steady_clock::now();
+    int rc;
+    try {
+        rc = setup(h, cell, atoms, shells, omega);
+    } catch (const std::bad_alloc &) {
+        rc = fail(h, PBC_JK_ERR_NOMEM, "host allocation failed");
+    } catch (...) {
+        rc = fail(h, PBC_JK_ERR_INVALID_ARG, "unexpected failure in setup");
+    }
+    if (rc != PBC_JK_OK) {
+        g_create_error = h->err;
+        h->pool.free_all();
+        for (auto &e : h->ev)
+            if (e) cudaEventDestroy(e);
+        delete h;
+        return rc;
+    }
+    h->create_seconds = std::chrono::duration<double>(std::chrono::steady_clock::now() - t0).count();
+    *out = h;
+    return PBC_JK_OK;
+}
+
+int pbc_jk_nbf(const pbc_jk *h) { return h ? h->N : PBC_JK_ERR_INVALID_ARG; }
+
+int pbc_jk_overlap(const pbc_jk *h, double *S_host)
+{
+    if (!h || !S_host) return PBC_JK_ERR_INVALID_ARG;
+    std::memcpy(S_host, h->S_host.data(), h->S_host.size() * sizeof(double));
+    return PBC_JK_OK;
+}
+
+int pbc_jk_set_parts(pbc_jk *h, int32_t parts)
+{
+    if (!h || parts < 0 || parts > 7) return PBC_JK_ERR_INVALID_ARG;
+    h->parts = parts;
+    return PBC_JK_OK;
+}
+
+int pbc_jk_build(pbc_jk *h, const double *P, double *J, double *K, void *cuda_stream)
+{
+    if (!h) return PBC_JK_ERR_INVALID_ARG;
+    if (!P) return fail(h, PBC_JK_ERR_INVALID_ARG, "P is null");
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const int N = h->N, Np = h->Np;
+    const size_t NN = (size_t)N * N;
+    const bool doSR = h->parts & 1, doLR = h->parts & 2, doSELF = h->parts & 4;
+    CK(cudaMemsetAsync(h->counters, 0, CNT_N * 8, st));
+    CK(cudaEventRecord(h->ev[0], st));
+    launch_scale_density(P, h->Pp, N, Np, h->fcomp, h->maxbits, h->lnPmax, st);
+    SRParams sp;
+    sp.K = h->K; sp.U = h->U; sp.KJ = h->KJ; sp.lat = h->lat; sp.sh = h->sh;
+    sp.boys = h->boys; sp.Pp = h->Pp; sp.ldP = Np; sp.Dt = h->Dt; sp.Jt = h->Jt; sp.Ksr = h->Ksr;
+    sp.lnPmax = h->lnPmax;
+    sp.ln_tau = std::log(h->cut.d_schwarz > 0 ? h->cut.d_schwarz : 1e-13);
+    sp.rcut2 = h->cut.r_cut > 0 ? h->cut.r_cut * h->cut.r_cut : std::numeric_limits<double>::infinity();
+    sp.counters = h->counters;
+    if (J && doSR) launch_hermite_density(h->U, h->sh, h->KJ, h->Pp, Np, h->Dt, st);
+    CK(cudaEventRecord(h->ev[1], st));
+    // ---- A5: real-space J ----
+    if (J && doSR) {
+        CK(cudaMemsetAsync(h->Jt, 0, (size_t)nherm(4) * std::max(h->U.n, 1) * 8, st));
+        CK(cudaMemsetAsync(h->Jsr, 0, NN * 8, st));
+        for (int LB = 0; LB <= 4; ++LB)
+            for (int LK = 0; LK <= 4; ++LK) launch_sr_j(LB, LK, sp, h->jbra[LB], h->njbra[LB], st);
+        launch_j_backtransform(h->U, h->sh, h->Jt, h->Jsr, N, st);
+    }
+    CK(cudaEventRecord(h->ev[2], st));
+    // ---- A6: real-space K ----
+    if (K && doSR) {
+        CK(cudaMemsetAsync(h->Ksr, 0, NN * 8, st));
+        for (int la = LMAX; la >= 0; --la)
+            for (int ld = la; ld >= 0; --ld)
+                for (int lb = LMAX; lb >= 0; --lb)
+                    for (int lc = LMAX; lc >= 0; --lc)
+                        launch_sr_k(la, lb, lc, ld, sp, h->kblk[la][ld], h->nkblk[la][ld], st);
+    }
+    CK(cudaEventRecord(h->ev[3], st));
+    // ---- A7/A8: reciprocal space, batches of G ----
+    const bool needJlr = J && (doLR || doSELF), needKlr = K && (doLR || doSELF);
+    if (needJlr) CK(cudaMemsetAsync(h->Jlr, 0, NN * 8, st));
+    if (needKlr) CK(cudaMemsetAsync(h->Klr, 0, (size_t)h->nsplit * Np * Np * 8, st));
+    const size_t strideK = (size_t)Np * Np;
+    if (doLR) {
+        for (int g0 = 0; g0 < h->nG; g0 += h->nb) {
+            const int nb = std::min(h->nb, h->nG - g0), nslot = 2 * nb;
+            launch_agen(h->lr, g0, nb, 0.0, h->Astack, h->ld, st);
+            if (J) {
+                launch_rho_reduce(h->Pp, h->Astack, h->ld, Np, N, nslot, h->rho, st);
+                launch_jlr_accum(h->Astack, h->ld, Np, N, nslot, h->rho, 1.0, h->Jlr, st);
+            }
+            if (K) {
+                // Z = P' [A'_1 A'_2 ...]
+                launch_dgemm(Np, nslot * Np, Np, 1, 1.0, h->Pp, Np, 0, h->Astack, h->ld, 0, 0.0, h->Zstack, h->ld, 0, 1, st);
+                // K += sum_slot A'_slot Z_slot
+                launch_dgemm(Np, Np, Np, nslot, 1.0, h->Astack, h->ld, Np, h->Zstack, h->ld, Np, 1.0, h->Klr, Np, strideK,
+                             std::min(h->nsplit, nslot), st);
+            }
+        }
+    }
+    // ---- A9: the G = 0 slot, weight -pi/(Omega w^2), A = S ----
+    if (doSELF) {
+        launch_agen(h->lr, -1, 1, std::sqrt(h->c0), h->Astack, h->ld, st);
+        if (J) {
+            launch_rho_reduce(h->Pp, h->Astack, h->ld, Np, N, 1, h->rho, st);
+            launch_jlr_accum(h->Astack, h->ld, Np, N, 1, h->rho, -1.0, h->Jlr, st);
+        }
+        if (K) {
+            launch_dgemm(Np, Np, Np, 1, 1.0, h->Pp, Np, 0, h->Astack, h->ld, 0, 0.0, h->Zstack, h->ld, 0, 1, st);
+            launch_dgemm(Np, Np, Np, 1, -1.0, h->Astack, h->ld, 0, h->Zstack, h->ld, 0, 1.0, h->Klr, Np, strideK, 1, st);
+        }
+    }
+    CK(cudaEventRecord(h->ev[4], st));
+    // ---- A10 ----
+    if (J) launch_finalize_j(doSR ? h->Jsr : nullptr, needJlr ? h->Jlr : nullptr, N, h->fcomp, J, st);
+    if (K)
+        launch_finalize_k(doSR ? h->Ksr : nullptr, h->sh, needKlr ? h->Klr : nullptr, h->nsplit, strideK, Np, N, h->fcomp,
+                          h->shell_of_ao, K, st);
+    CK(cudaEventRecord(h->ev[5], st));
+    CK(cudaGetLastError());
+    h->last_stream = st;
+    h->built = true;
+    return PBC_JK_OK;
+}
+
+int pbc_jk_build_host(pbc_jk *h, const double *P_host, double *J_host, double *K_host)
+{
+    if (!h) return PBC_JK_ERR_INVALID_ARG;
+    if (!P_host) return fail(h, PBC_JK_ERR_INVALID_ARG, "P is null");
+    const size_t bytes = (size_t)h->N * h->N * 8;
+    CK(cudaMemcpyAsync(h->hostP, P_host, bytes, cudaMemcpyHostToDevice, 0));
+    const int rc = pbc_jk_build(h, h->hostP, J_host ? h->hostJ : nullptr, K_host ? h->hostK : nullptr, nullptr);
+    if (rc != PBC_JK_OK) return rc;
+    if (J_host) CK(cudaMemcpyAsync(J_host, h->hostJ, bytes, cudaMemcpyDeviceToHost, 0));
+    if (K_host) CK(cudaMemcpyAsync(K_host, h->hostK, bytes, cudaMemcpyDeviceToHost, 0));
+    CK(cudaStreamSynchronize(0));
+    return PBC_JK_OK;
+}
+
+int pbc_jk_get_stats(pbc_jk *h, pbc_jk_stats_t *out)
+{
+    if (!h || !out) return PBC_JK_ERR_INVALID_ARG;
+    std::memset(out, 0, sizeof(*out));
+    out->nbf = h->N; out->nshell = h->nshell; out->natom = h->natom; out->n_g = h->nG;
+    out->n_prim_pairs = h->n_prim_pairs; out->n_shell_pair_images = h->n_sp_images;
+    out->create_seconds = h->create_seconds;
+    if (h->built) {
+        CK(cudaEventSynchronize(h->ev[5]));
+        unsigned long long c[CNT_N];
+        CK(cudaMemcpy(c, h->counters, sizeof(c), cudaMemcpyDeviceToHost));
+        out->candidates_j = (int64_t)c[CNT_CAND_J]; out->quartets_j = (int64_t)c[CNT_Q_J];
+        out->candidates_k = (int64_t)c[CNT_CAND_K]; out->quartets_k = (int64_t)c[CNT_Q_K];
+        float ms[5];
+        for (int i = 0; i < 5; ++i) CK(cudaEventElapsedTime(&ms[i], h->ev[i], h->ev[i + 1]));
+        float tot;
+        CK(cudaEventElapsedTime(&tot, h->ev[0], h->ev[5]));
+        out->ms_density = ms[0]; out->ms_sr_j = ms[1]; out->ms_sr_k = ms[2]; out->ms_lr = ms[3] + ms[4]; out->ms_total = tot;
+    }
+    return PBC_JK_OK;
+}
+
+const char *pbc_jk_last_error(const pbc_jk *h) { return h ? h->err.c_str() : g_create_error.c_str(); }
+
+int pbc_jk_destroy(pbc_jk *h)
+{
+    if (!h) return PBC_JK_OK;
+    cudaDeviceSynchronize();
+    h->pool.free_all();
+    for (auto &e : h->ev)
+        if (e) cudaEventDestroy(e);
+    delete h;
+    return PBC_JK_OK;
+}
+
+int pbc_jk_fp64_peak(int32_t iters, double *tflops_out)
+{
+    if (!tflops_out || iters < 1) return PBC_JK_ERR_INVALID_ARG;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
+        cudaGetLastError();
+        return PBC_JK_ERR_CUDA;
+    }
+    const double v = run_fp64_peak(iters);
+    if (v < 0) return PBC_JK_ERR_CUDA;
+    *tflops_out = v;
+    return PBC_JK_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,82 @@
+// Internal data model of libpbc_jk (host setup <-> kernels).  Not part of the C ABI.
+//
+// Notation follows PAPER.md / SURVEY.md 8: primitive pair-image (a in shell A at its home position,
+// b in shell B translated by R2): p = a+b, P = (aA + b(B+R2))/p (L131), coefficient
+//   coef = c_a c_b N_a N_b exp(-ab/p |A-B-R2|^2) * sqrt(2) pi^{5/4} / p
+// so that the eq-55 prefactor 2 pi^{5/2}/(p q sqrt(p+q)) of a quartet is coef_bra*coef_ket/sqrt(p+q).
+// N_a is the eq-6 norm of the AXIS-ALIGNED component (x^l); the remaining per-component factor
+// (sqrt(3) for d_xy, d_xz, d_yz) is folded into P on input and into J, K on output.
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+namespace pbcjk {
+
+constexpr int LMAX = 2;                 // s, p, d
+constexpr int LTOT = 4 * LMAX;          // highest Hermite order of a quartet
+constexpr int BOYS_NT = 8;              // Taylor terms (degree 7)
+constexpr int BOYS_MCOL = 16;           // F_0..F_15 per table row = one 128-byte line
+constexpr double BOYS_DX = 0.125;       // grid spacing
+constexpr double BOYS_XMAX = 36.0;      // beyond: asymptotic form
+constexpr int BOYS_ROWS = 289;          // 0, 1/8, ..., 36
+
+__host__ __device__ constexpr int ncart(int l) { return (l + 1) * (l + 2) / 2; }
+__host__ __device__ constexpr int nherm(int L) { return (L + 1) * (L + 2) * (L + 3) / 6; }
+// flat index of Hermite (t,u,v): orders ascending; inside an order the Cartesian component order
+// xx,xy,xz,yy,yz,zz.  hidx(t,u,v) - nherm(n-1) is the component index of a shell l = n.
+__host__ __device__ constexpr int hidx(int t, int u, int v)
+{
+    int n = t + u + v;
+    return n * (n + 1) * (n + 2) / 6 + (n - t) * (n - t + 1) / 2 + (n - t - u);
+}
+
+// ---- ordered primitive pair-images, sorted by (shell A, l of shell B, bound descending): K lists ----
+struct PairListK {
+    int n;
+    const double *Px, *Py, *Pz, *p, *ip, *coef, *lb; // ip = 1/p, lb = ln(bound)
+    const double *PAx, *PAy, *PAz, *PBx, *PBy, *PBz; // P - A, P - (B + R2)
+    const int *aoB;                                  // AO offset of shell B
+    const int *off;                                  // [nshell*3 + 1]: range of (A, lB)
+    const double *ext;                               // [nshell*3]: max |P - A| in the range
+    const double *ipmax;                             // [nshell*3]: max 1/p in the range
+};
+
+// ---- unordered primitive pair-images (shell A >= shell B), contiguous per shell pair ----
+struct PairListU {
+    int n, nsp;
+    const double *Px, *Py, *Pz, *p, *ip, *coef, *lb;
+    const double *PAx, *PAy, *PAz, *PBx, *PBy, *PBz;
+    const int *sp;                                   // shell-pair index of each entry
+    const int *sp_off;                               // [nsp + 1]
+    const int *sp_shA, *sp_shB;                      // [nsp]
+};
+
+// ---- J kets: U entries regrouped by (atom of shell A, Hermite order Lk, bound descending) ----
+struct KetListJ {
+    int n, ngroup;                                   // ngroup = natom
+    const double *Qx, *Qy, *Qz, *q, *iq, *coef, *lb;
+    const int *uidx;                                 // index into U
+    const int *off;                                  // [natom*5 + 1]
+    const double *ext, *iqmax;                       // [natom*5]
+    const double *gx, *gy, *gz;                      // [natom] group centre (atom position)
+    int64_t dstride;                                 // D~[s*dstride + j]
+};
+
+struct Lattice {
+    double a[9];        // rows a1,a2,a3
+    double binv[9];     // f = binv * r  (fractional coordinates, rows = b_i / 2pi)
+    double bnorm[3];    // |b_i| / 2pi   (half-width of the bounding box per unit radius, eq 99-103)
+    double omega, omega2, iomega2;
+    double volume;
+};
+
+struct ShellInfo {
+    const int *l, *ao, *atom;       // [nshell]
+    const double *cx, *cy, *cz;     // shell centre
+    int nshell, nbf;
+};
+
+// counters (device, int64): 0 cand_j, 1 quart_j, 2 cand_k, 3 quart_k
+enum { CNT_CAND_J = 0, CNT_Q_J = 1, CNT_CAND_K = 2, CNT_Q_K = 3, CNT_N = 8 };
+
+}  // namespace pbcjk

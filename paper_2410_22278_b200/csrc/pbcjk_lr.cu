@@ -1,0 +1,496 @@
+// Light kernels around the quartet kernels, and the reciprocal-space path.
+//
+//   rho_mn(G) = sum_{R2,prims} C_m C_n (pi/p)^{3/2} e^{-G^2/4p} e^{-iG.P} sum_t E^{mn}_t (-iG)^t
+//   J^LR_mn   = sum_{G != 0} w(G) Re[conj(rho_mn(G)) rho(G)],  rho(G) = sum_ls P_ls rho_ls(G)   (eq 98 first term)
+//   K^LR_mn   = sum_{G != 0} w(G) Re[sum_ls conj(rho_ml(G)) P_ls rho_sn(G)]
+//             = sum_G w (Ar P Ar + Ai P Ai)      since rho_mn(G) = Ar + i Ai is symmetric in (m,n) at Gamma
+//   SELF      = the G = 0 slot with weight -pi/(Omega w^2) and A = S                           (eq 35, eq 56 third term)
+// Half sphere of G, +-G paired (factor 2 in w, L243).  A' = sqrt(w) A is stored so both GEMM
+// operands carry the weight.  The K contraction is a dense FP64 GEMM over (G, lambda): it runs on
+// the FP64 tensor cores (DMMA, mma.sync.m8n8k4.f64) -- tcgen05 has no f64 kind.
+#include "pbcjk_lr.cuh"
+#include "pbcjk_md.cuh"
+#include <cmath>
+
+namespace pbcjk {
+
+// ---------------------------------------------------------------- density prep (A4)
+__global__ void scale_density_kernel(const double *__restrict__ P, double *__restrict__ Pp, int N, int Np,
+                                     const double *__restrict__ f, unsigned long long *maxbits)
+{
+    const size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    double v = 0.0;
+    if (idx < (size_t)N * N) {
+        const int i = (int)(idx / N), j = (int)(idx % N);
+        v = P[idx] * f[i] * f[j];
+        Pp[(size_t)i * Np + j] = v;
+        v = fabs(v);
+    }
+    // block maximum; one atomic per block (not on the quartet path)
+    __shared__ double s[32];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, o));
+    if ((threadIdx.x & 31) == 0) s[threadIdx.x >> 5] = v;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double m = 0.0;
+        for (int w = 0; w < (int)(blockDim.x >> 5); ++w) m = fmax(m, s[w]);
+        atomicMax(maxbits, (unsigned long long)__double_as_longlong(m));
+    }
+}
+__global__ void lnpmax_kernel(const unsigned long long *maxbits, double *lnPmax)
+{
+    double m = __longlong_as_double((long long)*maxbits);
+    *lnPmax = log(fmax(m, 1e-300));
+}
+void launch_scale_density(const double *P, double *Pp, int N, int Np, const double *fcomp,
+                          unsigned long long *maxbits, double *lnPmax, cudaStream_t st)
+{
+    cudaMemsetAsync(maxbits, 0, sizeof(unsigned long long), st);
+    const size_t tot = (size_t)N * N;
+    scale_density_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, st>>>(P, Pp, N, Np, fcomp, maxbits);
+    lnpmax_kernel<<<1, 1, 0, st>>>(maxbits, lnPmax);
+}
+
+// Hermite density of a ket primitive pair-image: D~_s = fac * sum_{cd} E^{cd}_s P'_cd   (eq 95)
+// fac = 2 for shell(C) != shell(D): the pair (D, C - R3) is the same distribution translated.
+__global__ void hermite_density_kernel(PairListU U, ShellInfo sh, KetListJ KJ, const double *__restrict__ Pp, int Np,
+                                       double *__restrict__ Dt)
+{
+    const int j = blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= KJ.n) return;
+    const int u = KJ.uidx[j];
+    const int sp = U.sp[u];
+    const int A = U.sp_shA[sp], B = U.sp_shB[sp];
+    const int la = sh.l[A], lb = sh.l[B];
+    const double o2p = 0.5 * U.ip[u];
+    E1Drt ex, ey, ez;
+    ex.build(la, lb, U.PAx[u], U.PBx[u], o2p);
+    ey.build(la, lb, U.PAy[u], U.PBy[u], o2p);
+    ez.build(la, lb, U.PAz[u], U.PBz[u], o2p);
+    double D[nherm(2 * LMAX)];
+    const int L = la + lb, nh = nherm(L);
+    for (int s = 0; s < nh; ++s) D[s] = 0.0;
+    const int na = ncart(la), nb = ncart(lb);
+    const double *Pb = Pp + (size_t)sh.ao[A] * Np + sh.ao[B];
+    for (int a = 0; a < na; ++a)
+        for (int b = 0; b < nb; ++b) {
+            int ax, ay, az, bx, by, bz;
+            cart_powers(la, a, ax, ay, az);
+            cart_powers(lb, b, bx, by, bz);
+            const double pv = Pb[(size_t)a * Np + b];
+            for (int tx = 0; tx <= ax + bx; ++tx)
+                for (int ty = 0; ty <= ay + by; ++ty)
+                    for (int tz = 0; tz <= az + bz; ++tz)
+                        D[hidx(tx, ty, tz)] += pv * ex.e[ax][bx][tx] * ey.e[ay][by][ty] * ez.e[az][bz][tz];
+        }
+    const double fac = (A != B) ? 2.0 : 1.0;
+    for (int s = 0; s < nh; ++s) Dt[(size_t)s * KJ.dstride + j] = fac * D[s];
+}
+void launch_hermite_density(const PairListU &U, const ShellInfo &sh, const KetListJ &KJ, const double *Pp, int Np,
+                            double *Dt, cudaStream_t st)
+{
+    if (KJ.n <= 0) return;
+    hermite_density_kernel<<<(KJ.n + 127) / 128, 128, 0, st>>>(U, sh, KJ, Pp, Np, Dt);
+}
+
+// J_ab = sum_{R2,prims} sum_t (-1)^{|t|} E^{ab}_t J_t  (eq 96-97); one warp per shell pair.
+__global__ void j_backtransform_kernel(PairListU U, ShellInfo sh, const double *__restrict__ Jt, double *__restrict__ Jsr,
+                                       int N)
+{
+    const int sp = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    const int lane = threadIdx.x & 31;
+    if (sp >= U.nsp) return;
+    const int A = U.sp_shA[sp], B = U.sp_shB[sp];
+    const int la = sh.l[A], lb = sh.l[B];
+    const int na = ncart(la), nb = ncart(lb);
+    double acc[36];
+    for (int i = 0; i < 36; ++i) acc[i] = 0.0;
+    for (int u = U.sp_off[sp] + lane; u < U.sp_off[sp + 1]; u += 32) {
+        const double o2p = 0.5 * U.ip[u];
+        E1Drt ex, ey, ez;
+        ex.build(la, lb, U.PAx[u], U.PBx[u], o2p);
+        ey.build(la, lb, U.PAy[u], U.PBy[u], o2p);
+        ez.build(la, lb, U.PAz[u], U.PBz[u], o2p);
+        for (int a = 0; a < na; ++a)
+            for (int b = 0; b < nb; ++b) {
+                int ax, ay, az, bx, by, bz;
+                cart_powers(la, a, ax, ay, az);
+                cart_powers(lb, b, bx, by, bz);
+                double s = 0.0;
+                for (int tx = 0; tx <= ax + bx; ++tx)
+                    for (int ty = 0; ty <= ay + by; ++ty)
+                        for (int tz = 0; tz <= az + bz; ++tz) {
+                            double e = ex.e[ax][bx][tx] * ey.e[ay][by][ty] * ez.e[az][bz][tz];
+                            if ((tx + ty + tz) & 1) e = -e;                       // reading C-4
+                            s += e * Jt[(size_t)hidx(tx, ty, tz) * U.n + u];
+                        }
+                acc[a * nb + b] += s;
+            }
+    }
+    for (int i = 0; i < na * nb; ++i) {
+        double v = acc[i];
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+        if (lane == 0) {
+            const int a = i / nb, b = i % nb;
+            Jsr[(size_t)(sh.ao[A] + a) * N + sh.ao[B] + b] = v;
+            if (A != B) Jsr[(size_t)(sh.ao[B] + b) * N + sh.ao[A] + a] = v;
+        }
+    }
+}
+void launch_j_backtransform(const PairListU &U, const ShellInfo &sh, const double *Jt, double *Jsr, int N,
+                            cudaStream_t st)
+{
+    if (U.nsp <= 0) return;
+    j_backtransform_kernel<<<(U.nsp + 3) / 4, 128, 0, st>>>(U, sh, Jt, Jsr, N);
+}
+
+// ---------------------------------------------------------------- rho_mn(G) generation (A7)
+// thread = (shell pair, G of the batch).  Writes the block and its mirror (rho_mn = rho_nm).
+__global__ void agen_kernel(LRParams p, int g0, int nb, double w0, double *__restrict__ Astack, size_t ld)
+{
+    const int sp = blockIdx.x;
+    const int gl = blockIdx.y * blockDim.x + threadIdx.x;
+    if (gl >= nb) return;
+    const bool overlap = g0 < 0;
+    double Gx = 0, Gy = 0, Gz = 0, sw = w0;
+    if (!overlap) {
+        Gx = p.Gx[g0 + gl]; Gy = p.Gy[g0 + gl]; Gz = p.Gz[g0 + gl]; sw = p.Gw[g0 + gl];
+    }
+    const double G2 = Gx * Gx + Gy * Gy + Gz * Gz;
+    const PairListU &U = p.U;
+    const int A = U.sp_shA[sp], B = U.sp_shB[sp];
+    const int la = p.sh.l[A], lb = p.sh.l[B];
+    const int na = ncart(la), nbc = ncart(lb);
+    double accr[36], acci[36];
+    for (int i = 0; i < 36; ++i) { accr[i] = 0.0; acci[i] = 0.0; }
+    for (int u = U.sp_off[sp]; u < U.sp_off[sp + 1]; ++u) {
+        const double pp = U.p[u], ip = U.ip[u];
+        // coef holds sqrt2 pi^{5/4}/p; the transform needs (pi/p)^{3/2}
+        const double cft = U.coef[u] * 0.94139626377671481 * rsqrt(pp) * exp(-0.25 * G2 * ip) * sw;
+        double sn, cs;
+        sincos(-(Gx * U.Px[u] + Gy * U.Py[u] + Gz * U.Pz[u]), &sn, &cs);
+        const double phr = cft * cs, phi = cft * sn;
+        E1Drt ex, ey, ez;
+        const double o2p = 0.5 * ip;
+        ex.build(la, lb, U.PAx[u], U.PBx[u], o2p);
+        ey.build(la, lb, U.PAy[u], U.PBy[u], o2p);
+        ez.build(la, lb, U.PAz[u], U.PBz[u], o2p);
+        // per direction: S[i][j] = sum_t E^{ij}_t (-iG)^t
+        double sr[3][LMAX + 1][LMAX + 1], si[3][LMAX + 1][LMAX + 1];
+        for (int d = 0; d < 3; ++d) {
+            const E1Drt &e = d == 0 ? ex : (d == 1 ? ey : ez);
+            const double g = d == 0 ? Gx : (d == 1 ? Gy : Gz);
+            for (int i = 0; i <= la; ++i)
+                for (int j = 0; j <= lb; ++j) {
+                    double r = 0.0, im = 0.0, gp = 1.0;
+                    for (int t = 0; t <= i + j; ++t) {
+                        const double v = e.e[i][j][t] * gp;        // (-i)^t: 1, -i, -1, i
+                        switch (t & 3) {
+                        case 0: r += v; break;
+                        case 1: im -= v; break;
+                        case 2: r -= v; break;
+                        default: im += v; break;
+                        }
+                        gp *= g;
+                    }
+                    sr[d][i][j] = r; si[d][i][j] = im;
+                }
+        }
+        for (int a = 0; a < na; ++a)
+            for (int b = 0; b < nbc; ++b) {
+                int ax, ay, az, bx, by, bz;
+                cart_powers(la, a, ax, ay, az);
+                cart_powers(lb, b, bx, by, bz);
+                double r = sr[0][ax][bx], im = si[0][ax][bx];
+                double r2 = r * sr[1][ay][by] - im * si[1][ay][by], i2 = r * si[1][ay][by] + im * sr[1][ay][by];
+                r = r2 * sr[2][az][bz] - i2 * si[2][az][bz];
+                im = r2 * si[2][az][bz] + i2 * sr[2][az][bz];
+                accr[a * nbc + b] += r * phr - im * phi;
+                acci[a * nbc + b] += r * phi + im * phr;
+            }
+    }
+    const int oa = p.sh.ao[A], ob = p.sh.ao[B];
+    const size_t slot_r = overlap ? 0 : (size_t)(2 * gl), slot_i = slot_r + 1;
+    for (int a = 0; a < na; ++a)
+        for (int b = 0; b < nbc; ++b) {
+            const double vr = accr[a * nbc + b], vi = acci[a * nbc + b];
+            Astack[(size_t)(oa + a) * ld + slot_r * p.Np + ob + b] = vr;
+            Astack[(size_t)(ob + b) * ld + slot_r * p.Np + oa + a] = vr;
+            if (!overlap) {
+                Astack[(size_t)(oa + a) * ld + slot_i * p.Np + ob + b] = vi;
+                Astack[(size_t)(ob + b) * ld + slot_i * p.Np + oa + a] = vi;
+            }
+        }
+}
+void launch_agen(const LRParams &p, int g0, int nb, double w0, double *Astack, size_t ld, cudaStream_t st)
+{
+    if (p.U.nsp <= 0 || nb <= 0) return;
+    const int bs = nb >= 64 ? 64 : 32;
+    dim3 grid(p.U.nsp, (nb + bs - 1) / bs);
+    agen_kernel<<<grid, bs, 0, st>>>(p, g0, nb, w0, Astack, ld);
+}
+
+// rho'[slot] = sum_{mn} P'_mn A'_mn[slot]   (fixed-order block reduction => deterministic)
+__global__ void rho_reduce_kernel(const double *__restrict__ Pp, const double *__restrict__ Astack, size_t ld, int Np, int N,
+                                  double *__restrict__ rho)
+{
+    const int slot = blockIdx.x;
+    double acc = 0.0;
+    for (int i = threadIdx.x >> 5; i < N; i += (blockDim.x >> 5)) {
+        const double *a = Astack + (size_t)i * ld + (size_t)slot * Np;
+        const double *pr = Pp + (size_t)i * Np;
+        for (int j = threadIdx.x & 31; j < N; j += 32) acc = fma(pr[j], a[j], acc);
+    }
+    __shared__ double s[32];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+    if ((threadIdx.x & 31) == 0) s[threadIdx.x >> 5] = acc;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double t = 0.0;
+        for (int w = 0; w < (int)(blockDim.x >> 5); ++w) t += s[w];
+        rho[slot] = t;
+    }
+}
+void launch_rho_reduce(const double *Pp, const double *Astack, size_t ld, int Np, int N, int nslot, double *rho,
+                       cudaStream_t st)
+{
+    if (nslot <= 0) return;
+    rho_reduce_kernel<<<nslot, 512, 0, st>>>(Pp, Astack, ld, Np, N, rho);
+}
+
+__global__ void jlr_accum_kernel(const double *__restrict__ Astack, size_t ld, int Np, int N, int nslot,
+                                 const double *__restrict__ rho, double sign, double *__restrict__ Jacc)
+{
+    const int n = blockIdx.x * blockDim.x + threadIdx.x, m = blockIdx.y;
+    if (n >= N) return;
+    const double *a = Astack + (size_t)m * ld + n;
+    double acc = 0.0;
+    for (int s = 0; s < nslot; ++s) acc = fma(a[(size_t)s * Np], rho[s], acc);
+    Jacc[(size_t)m * N + n] += sign * acc;
+}
+void launch_jlr_accum(const double *Astack, size_t ld, int Np, int N, int nslot, const double *rho, double sign,
+                      double *Jacc, cudaStream_t st)
+{
+    if (nslot <= 0) return;
+    dim3 grid((N + 127) / 128, N);
+    jlr_accum_kernel<<<grid, 128, 0, st>>>(Astack, ld, Np, N, nslot, rho, sign, Jacc);
+}
+
+// ---------------------------------------------------------------- FP64 tensor-core GEMM (A8, A9)
+namespace {
+constexpr int BM = 128, BN = 128, BK = 16;
+constexpr int SA = BK + 4;    // row stride of the A tile [m][k]: (lane/4)*20 + lane%4 hits every bank pair twice
+constexpr int SB = BN + 8;    // row stride of the B tile [k][n]: (lane%4)*136 + lane/4 likewise
+constexpr int GEMM_SMEM = 2 * (BM * SA + BK * SB) * (int)sizeof(double);
+
+__device__ __forceinline__ void cp_async16(void *smem, const void *gmem)
+{
+    unsigned s = (unsigned)__cvta_generic_to_shared(smem);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(s), "l"(gmem));
+}
+__device__ __forceinline__ void dmma(double &c0, double &c1, double a, double b)
+{
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
+                 : "+d"(c0), "+d"(c1)
+                 : "d"(a), "d"(b));
+}
+}  // namespace
+
+__global__ void __launch_bounds__(256) dgemm_kernel(int Kb, int nbatch, double alpha, const double *__restrict__ A, size_t lda,
+                                                    size_t strideA, const double *__restrict__ B, size_t ldb, size_t strideB,
+                                                    double beta, double *__restrict__ C, size_t ldc, size_t strideC, int nsplit)
+{
+    extern __shared__ __align__(16) double smem[];
+    double *As = smem;                       // [2][BM*SA]
+    double *Bs = smem + 2 * BM * SA;         // [2][BK*SB]
+    const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
+    const int wm = w >> 2, wn = w & 3;
+    const int bm = blockIdx.y, bn = blockIdx.x, z = blockIdx.z;
+    const int bat0 = (int)((long long)nbatch * z / nsplit), bat1 = (int)((long long)nbatch * (z + 1) / nsplit);
+    const int kt_per = Kb / BK;
+    const int ntile = (bat1 - bat0) * kt_per;
+    C += (size_t)z * strideC;
+
+    double acc[8][4][2];
+#pragma unroll
+    for (int i = 0; i < 8; ++i)
+#pragma unroll
+        for (int j = 0; j < 4; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
+
+    auto load_tile = [&](int t, int buf) {
+        const int b = bat0 + t / kt_per, k0 = (t % kt_per) * BK;
+        const double *Ab = A + (size_t)b * strideA + (size_t)(bm * BM) * lda + k0;
+        const double *Bb = B + (size_t)b * strideB + (size_t)k0 * ldb + bn * BN;
+        double *as = As + buf * BM * SA, *bs = Bs + buf * BK * SB;
+#pragma unroll
+        for (int c = tid; c < BM * BK / 2; c += 256) {
+            const int row = c >> 3, c2 = c & 7;
+            cp_async16(as + row * SA + c2 * 2, Ab + (size_t)row * lda + c2 * 2);
+        }
+#pragma unroll
+        for (int c = tid; c < BK * BN / 2; c += 256) {
+            const int row = c >> 6, c2 = c & 63;
+            cp_async16(bs + row * SB + c2 * 2, Bb + (size_t)row * ldb + c2 * 2);
+        }
+        asm volatile("cp.async.commit_group;\n" ::);
+    };
+
+    if (ntile > 0) load_tile(0, 0);
+    for (int t = 0; t < ntile; ++t) {
+        const int buf = t & 1;
+        if (t + 1 < ntile) {
+            load_tile(t + 1, buf ^ 1);
+            asm volatile("cp.async.wait_group 1;\n" ::);
+        } else {
+            asm volatile("cp.async.wait_group 0;\n" ::);
+        }
+        __syncthreads();
+        const double *as = As + buf * BM * SA + (wm * 64 + (lane >> 2)) * SA + (lane & 3);
+        const double *bs = Bs + buf * BK * SB + (lane & 3) * SB + wn * 32 + (lane >> 2);
+#pragma unroll
+        for (int kk = 0; kk < BK; kk += 4) {
+            double a[8], b[4];
+#pragma unroll
+            for (int i = 0; i < 8; ++i) a[i] = as[i * 8 * SA + kk];
+#pragma unroll
+            for (int j = 0; j < 4; ++j) b[j] = bs[kk * SB + j * 8];
+#pragma unroll
+            for (int i = 0; i < 8; ++i)
+#pragma unroll
+                for (int j = 0; j < 4; ++j) dmma(acc[i][j][0], acc[i][j][1], a[i], b[j]);
+        }
+        __syncthreads();
+    }
+#pragma unroll
+    for (int i = 0; i < 8; ++i)
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const size_t row = (size_t)bm * BM + wm * 64 + i * 8 + (lane >> 2);
+            const size_t col = (size_t)bn * BN + wn * 32 + j * 8 + (lane & 3) * 2;
+            double2 *dst = reinterpret_cast<double2 *>(C + row * ldc + col);
+            double2 v = make_double2(alpha * acc[i][j][0], alpha * acc[i][j][1]);
+            if (beta != 0.0) {
+                const double2 o = *dst;
+                v.x = fma(beta, o.x, v.x);
+                v.y = fma(beta, o.y, v.y);
+            }
+            *dst = v;
+        }
+}
+
+void launch_dgemm(int M, int Nc, int Kb, int nbatch, double alpha, const double *A, size_t lda, size_t strideA,
+                  const double *B, size_t ldb, size_t strideB, double beta, double *C, size_t ldc, size_t strideC,
+                  int nsplit, cudaStream_t st)
+{
+    static bool attr_set = false;
+    if (!attr_set) {
+        cudaFuncSetAttribute(dgemm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, GEMM_SMEM);
+        attr_set = true;
+    }
+    dim3 grid(Nc / BN, M / BM, nsplit);
+    dgemm_kernel<<<grid, 256, GEMM_SMEM, st>>>(Kb, nbatch, alpha, A, lda, strideA, B, ldb, strideB, beta, C, ldc, strideC,
+                                               nsplit);
+}
+
+// ---------------------------------------------------------------- finalise (A10)
+__global__ void finalize_j_kernel(const double *__restrict__ Jsr, const double *__restrict__ Jlr, int N,
+                                  const double *__restrict__ f, double *__restrict__ J)
+{
+    const int n = blockIdx.x * blockDim.x + threadIdx.x, m = blockIdx.y;
+    if (n >= N) return;
+    double v = 0.0;
+    if (Jsr) v += 0.5 * (Jsr[(size_t)m * N + n] + Jsr[(size_t)n * N + m]);
+    if (Jlr) v += 0.5 * (Jlr[(size_t)m * N + n] + Jlr[(size_t)n * N + m]);
+    J[(size_t)m * N + n] = f[m] * f[n] * v;
+}
+void launch_finalize_j(const double *Jsr, const double *Jlr, int N, const double *fcomp, double *J, cudaStream_t st)
+{
+    dim3 grid((N + 127) / 128, N);
+    finalize_j_kernel<<<grid, 128, 0, st>>>(Jsr, Jlr, N, fcomp, J);
+}
+
+// K_sr holds the blocks (mu, nu) with l_mu > l_nu, or l_mu == l_nu and mu >= nu; the rest by K = K^T.
+__global__ void finalize_k_kernel(const double *__restrict__ Ksr, ShellInfo sh, const double *__restrict__ Klr, int nsplit,
+                                  size_t strideK, int Np, int N, const double *__restrict__ f,
+                                  const int *__restrict__ shell_of_ao, double *__restrict__ K)
+{
+    const int n = blockIdx.x * blockDim.x + threadIdx.x, m = blockIdx.y;
+    if (n >= N) return;
+    double v = 0.0;
+    if (Ksr) {
+        const int sm = shell_of_ao[m], sn = shell_of_ao[n];
+        const int lm = sh.l[sm], ln = sh.l[sn];
+        if (sm == sn) v = 0.5 * (Ksr[(size_t)m * N + n] + Ksr[(size_t)n * N + m]);
+        else if (lm > ln || (lm == ln && sm > sn)) v = Ksr[(size_t)m * N + n];
+        else v = Ksr[(size_t)n * N + m];
+    }
+    if (Klr) {
+        double t = 0.0;
+        for (int z = 0; z < nsplit; ++z)
+            t += Klr[z * strideK + (size_t)m * Np + n] + Klr[z * strideK + (size_t)n * Np + m];
+        v += 0.5 * t;
+    }
+    K[(size_t)m * N + n] = f[m] * f[n] * v;
+}
+void launch_finalize_k(const double *Ksr, const ShellInfo &sh, const double *Klr, int nsplit, size_t strideK, int Np,
+                       int N, const double *fcomp, const int *shell_of_ao, double *K, cudaStream_t st)
+{
+    dim3 grid((N + 127) / 128, N);
+    finalize_k_kernel<<<grid, 128, 0, st>>>(Ksr, sh, Klr, nsplit, strideK, Np, N, fcomp, shell_of_ao, K);
+}
+
+__global__ void extract_overlap_kernel(const double *__restrict__ Astack, size_t ld, int N, const double *__restrict__ f,
+                                       double *__restrict__ S)
+{
+    const int n = blockIdx.x * blockDim.x + threadIdx.x, m = blockIdx.y;
+    if (n >= N) return;
+    S[(size_t)m * N + n] = f[m] * f[n] * Astack[(size_t)m * ld + n];
+}
+void launch_extract_overlap(const double *Astack, size_t ld, int N, const double *fcomp, double *S, cudaStream_t st)
+{
+    dim3 grid((N + 127) / 128, N);
+    extract_overlap_kernel<<<grid, 128, 0, st>>>(Astack, ld, N, fcomp, S);
+}
+
+// ---------------------------------------------------------------- FP64 FMA peak (roofline denominator)
+__global__ void __launch_bounds__(256) fp64_peak_kernel(int iters, double *out)
+{
+    double a0 = threadIdx.x * 1e-9, a1 = a0 + 1, a2 = a0 + 2, a3 = a0 + 3, a4 = a0 + 4, a5 = a0 + 5, a6 = a0 + 6, a7 = a0 + 7;
+    const double b = 1.0000001, c = 1e-9;
+    for (int i = 0; i < iters; ++i) {
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+            a0 = fma(a0, b, c); a1 = fma(a1, b, c); a2 = fma(a2, b, c); a3 = fma(a3, b, c);
+            a4 = fma(a4, b, c); a5 = fma(a5, b, c); a6 = fma(a6, b, c); a7 = fma(a7, b, c);
+        }
+    }
+    const double s = a0 + a1 + a2 + a3 + a4 + a5 + a6 + a7;
+    if (s == 1.2345) out[0] = s;
+}
+double run_fp64_peak(int iters)
+{
+    int dev = 0, nsm = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
+    double *d = nullptr;
+    if (cudaMalloc(&d, 8) != cudaSuccess) return -1.0;
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0); cudaEventCreate(&e1);
+    const int blocks = nsm * 8;
+    fp64_peak_kernel<<<blocks, 256>>>(iters / 8 + 1, d);
+    cudaEventRecord(e0);
+    fp64_peak_kernel<<<blocks, 256>>>(iters, d);
+    cudaEventRecord(e1);
+    cudaEventSynchronize(e1);
+    float ms = 0;
+    cudaEventElapsedTime(&ms, e0, e1);
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    cudaFree(d);
+    if (cudaGetLastError() != cudaSuccess || ms <= 0) return -1.0;
+    const double flop = 2.0 * 64.0 * (double)iters * 256.0 * blocks;
+    return flop / (ms * 1e-3) * 1e-12;
+}
+
+}  // namespace pbcjk

@@ -1,0 +1,48 @@
+// Launchers of the "light" kernels: density prep (A4), J back-transform (eq 97), reciprocal-space
+// passes (A7-A9) and the FP64 tensor-core GEMM used by the reciprocal-space K contraction (A8).
+#pragma once
+#include "pbcjk_common.h"
+
+namespace pbcjk {
+
+struct LRParams {
+    PairListU U;
+    ShellInfo sh;
+    Lattice lat;
+    int N, Np;                 // basis size and its padded size (multiple of 128)
+    const double *fcomp;       // [N] per-component factor (1 or sqrt 3)
+    const double *Gx, *Gy, *Gz, *Gw;   // half-sphere G list, Gw = sqrt(2 * 4 pi/(Omega G^2) exp(-G^2/4w^2))
+};
+
+// P' = f P f (into the padded Np x Np buffer, pads untouched) and ln(max |P'|)
+void launch_scale_density(const double *P, double *Pp, int N, int Np, const double *fcomp,
+                          unsigned long long *maxbits, double *lnPmax, cudaStream_t st);
+// D~_s of every J ket (eq 95)
+void launch_hermite_density(const PairListU &U, const ShellInfo &sh, const KetListJ &KJ, const double *Pp, int Np,
+                            double *Dt, cudaStream_t st);
+// J_ab += sum_t (-1)^{|t|} E^{ab}_t Jt  per shell pair, mirrored (eq 96-97)
+void launch_j_backtransform(const PairListU &U, const ShellInfo &sh, const double *Jt, double *Jsr, int N,
+                            cudaStream_t st);
+// A'(G) = sqrt(w) rho_mn(G) for G in [g0, g0+nb): real and imaginary parts as 2*nb slots of the
+// stack  A[row*ld + slot*Np + col], ld = 2*nb_alloc*Np.  g0 < 0: the single G = 0 slot with
+// weight `w0` (overlap S, eq 21), written to slot 0.
+void launch_agen(const LRParams &p, int g0, int nb, double w0, double *Astack, size_t ld, cudaStream_t st);
+// rho'[slot] = sum P' o A'[slot]
+void launch_rho_reduce(const double *Pp, const double *Astack, size_t ld, int Np, int N, int nslot, double *rho,
+                       cudaStream_t st);
+// Jacc[m][n] += sign * sum_slot A'[slot][m][n] rho'[slot]
+void launch_jlr_accum(const double *Astack, size_t ld, int Np, int N, int nslot, const double *rho, double sign,
+                      double *Jacc, cudaStream_t st);
+// C[M x Nc] (ldc) = beta*C + alpha * sum_b A_b[M x Kb](lda) B_b[Kb x Nc](ldb); all dims multiples of
+// 128 (M, Nc) / 16 (Kb); grid.z = nsplit partial results C + z*strideC over disjoint batch ranges.
+void launch_dgemm(int M, int Nc, int Kb, int nbatch, double alpha, const double *A, size_t lda, size_t strideA,
+                  const double *B, size_t ldb, size_t strideB, double beta, double *C, size_t ldc, size_t strideC,
+                  int nsplit, cudaStream_t st);
+// out = f f (sum of parts), symmetrised; see pbcjk_lr.cu
+void launch_finalize_j(const double *Jsr, const double *Jlr, int N, const double *fcomp, double *J, cudaStream_t st);
+void launch_finalize_k(const double *Ksr, const ShellInfo &sh, const double *Klr, int nsplit, size_t strideK, int Np,
+                       int N, const double *fcomp, const int *shell_of_ao, double *K, cudaStream_t st);
+void launch_extract_overlap(const double *Astack, size_t ld, int N, const double *fcomp, double *S, cudaStream_t st);
+double run_fp64_peak(int iters);
+
+}  // namespace pbcjk
