@@ -84,7 +84,20 @@ typedef struct {
     int64_t candidates_j, candidates_k;     /* primitive quartet-images tested by the screen      */
     double  ms_density, ms_sr_j, ms_sr_k, ms_lr, ms_total;   /* device times, CUDA events         */
     double  create_seconds;                 /* host wall time of pbc_jk_create                    */
+    int64_t n_launches;                     /* CUDA kernels the last build launched               */
 } pbc_jk_stats_t;
+
+/* One real-space kernel class of the LAST build (one launch per class and build).
+ * kind 0: J-engine class, l[0] = Hermite order of the bra pair (l_mu + l_nu), l[1] = of the ket pair
+ *         (eq 96-98); kind 1: K class (l_mu l_lambda | l_sigma l_nu) in l[0..3] (eq 74).
+ * quartets / candidates: primitive quartet-images evaluated / tested (eq 67) by that launch.
+ * ms: device time of the launch (CUDA events on the build's stream); 0 unless profile mode is on. */
+typedef struct {
+    int32_t kind;
+    int32_t l[4];
+    int64_t quartets, candidates;
+    double  ms;
+} pbc_jk_class_stat;
 
 /*
  * A1-A3: validates, builds the reciprocal lattice and the half-sphere G list
@@ -119,6 +132,13 @@ int pbc_jk_set_parts(pbc_jk *h, int32_t parts);
 
 /* waits for the last build on its stream and fills the counters/times */
 int pbc_jk_get_stats(pbc_jk *h, pbc_jk_stats_t *out);
+
+/* profile mode (default off): record a CUDA event pair around every real-space class launch */
+int pbc_jk_set_profile(pbc_jk *h, int32_t on);
+
+/* waits for the last build and writes up to `cap` class records to `out` (HOST memory, caller-owned);
+ * *n_out = number of classes the build launched (may exceed cap: call again with a larger array) */
+int pbc_jk_get_class_stats(pbc_jk *h, pbc_jk_class_stat *out, int32_t cap, int32_t *n_out);
 
 /* text of the last error on this handle ("" if none); valid until the next call on the handle.
  * With h == NULL: the text of the last failed pbc_jk_create of this thread. */

@@ -20,7 +20,7 @@ STATUS = {0: "OK", -1: "INVALID_ARG", -2: "NOMEM", -3: "CUDA", -4: "UNSUPPORTED"
 
 # every symbol include/pbc_jk.h declares (checked by tests/test_abi.py)
 SYMBOLS = ["pbc_jk_create", "pbc_jk_nbf", "pbc_jk_overlap", "pbc_jk_build", "pbc_jk_build_host",
-           "pbc_jk_set_parts", "pbc_jk_get_stats", "pbc_jk_last_error", "pbc_jk_destroy", "pbc_jk_fp64_peak"]
+           "pbc_jk_set_parts", "pbc_jk_get_stats", "pbc_jk_set_profile", "pbc_jk_get_class_stats", "pbc_jk_last_error", "pbc_jk_destroy", "pbc_jk_fp64_peak"]
 
 
 class pbc_cell(C.Structure):
@@ -49,7 +49,12 @@ class pbc_jk_stats_t(C.Structure):
                 ("quartets_j", C.c_int64), ("quartets_k", C.c_int64),
                 ("candidates_j", C.c_int64), ("candidates_k", C.c_int64),
                 ("ms_density", C.c_double), ("ms_sr_j", C.c_double), ("ms_sr_k", C.c_double), ("ms_lr", C.c_double),
-                ("ms_total", C.c_double), ("create_seconds", C.c_double)]
+                ("ms_total", C.c_double), ("create_seconds", C.c_double), ("n_launches", C.c_int64)]
+
+
+class pbc_jk_class_stat(C.Structure):
+    _fields_ = [("kind", C.c_int32), ("l", C.c_int32 * 4), ("quartets", C.c_int64), ("candidates", C.c_int64),
+                ("ms", C.c_double)]
 
 
 _lib = None
@@ -78,6 +83,11 @@ def load() -> C.CDLL:
         lib.pbc_jk_set_parts.restype = C.c_int
         lib.pbc_jk_get_stats.argtypes = [C.c_void_p, C.POINTER(pbc_jk_stats_t)]
         lib.pbc_jk_get_stats.restype = C.c_int
+        lib.pbc_jk_set_profile.argtypes = [C.c_void_p, C.c_int32]
+        lib.pbc_jk_set_profile.restype = C.c_int
+        lib.pbc_jk_get_class_stats.argtypes = [C.c_void_p, C.POINTER(pbc_jk_class_stat), C.c_int32,
+                                               C.POINTER(C.c_int32)]
+        lib.pbc_jk_get_class_stats.restype = C.c_int
         lib.pbc_jk_last_error.argtypes = [C.c_void_p]
         lib.pbc_jk_last_error.restype = C.c_char_p
         lib.pbc_jk_destroy.argtypes = [C.c_void_p]
@@ -191,6 +201,23 @@ class PbcJK:
         s = pbc_jk_stats_t()
         self._check(load().pbc_jk_get_stats(self._h, C.byref(s)))
         return {f: getattr(s, f) for f, _ in s._fields_}
+
+    def set_profile(self, on: bool = True):
+        self._check(load().pbc_jk_set_profile(self._h, 1 if on else 0))
+
+    def class_stats(self) -> list:
+        """Per real-space kernel class of the last build: kind ('J'|'K'), l, quartets, candidates, ms."""
+        cap = 128
+        arr = (pbc_jk_class_stat * cap)()
+        n = C.c_int32()
+        self._check(load().pbc_jk_get_class_stats(self._h, arr, cap, C.byref(n)))
+        out = []
+        for i in range(min(n.value, cap)):
+            s = arr[i]
+            nl = 2 if s.kind == 0 else 4
+            out.append(dict(kind="J" if s.kind == 0 else "K", l=tuple(int(s.l[k]) for k in range(nl)),
+                            quartets=int(s.quartets), candidates=int(s.candidates), ms=float(s.ms)))
+        return out
 
     def close(self):
         if self._h:

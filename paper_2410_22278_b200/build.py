@@ -44,7 +44,8 @@ def _digest(src: str, defs) -> str:
     for f in [os.path.join(CSRC, src)] + [f if os.path.isabs(f) else os.path.join(CSRC, f) for f in HEADERS]:
         with open(f, "rb") as fh:
             h.update(fh.read())
-    h.update(" ".join(NVCC_FLAGS + list(defs)).encode())
+    # flags enter the key with the checkout path stripped: the objects built here stay valid on the GPU box
+    h.update(" ".join(NVCC_FLAGS + list(defs)).replace(os.path.dirname(HERE), ".").encode())
     return h.hexdigest()[:16]
 
 

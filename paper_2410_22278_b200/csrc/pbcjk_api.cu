@@ -81,9 +81,15 @@ struct pbc_jk {
     double *hostP = nullptr, *hostJ = nullptr, *hostK = nullptr;     // device staging of build_host
     unsigned long long *maxbits = nullptr, *counters = nullptr;
     int nb = 1, nsplit = 1;
+    bool has_l[LMAX + 1] = {};
     size_t ld = 0;
     double c0 = 0.0;             // pi/(Omega w^2)
     cudaEvent_t ev[6] = {};
+    // per-class events of the real-space launches (profile mode): [cls][start, stop]
+    cudaEvent_t evJ[NCLS_J][2] = {}, evK[NCLS_K][2] = {};
+    bool ranJ[NCLS_J] = {}, ranK[NCLS_K] = {};
+    bool profile = false;
+    int64_t n_launches = 0;
     cudaStream_t last_stream = nullptr;
     bool built = false;
     int64_t n_prim_pairs = 0, n_sp_images = 0;
@@ -171,6 +177,18 @@ void for_images_host(const Lattice &lat, const double c[3], double r, F &&f)
             }
 }
 
+void destroy_events(pbc_jk *h)
+{
+    for (auto &e : h->ev)
+        if (e) cudaEventDestroy(e);
+    for (auto &e : h->evJ)
+        for (auto &x : e)
+            if (x) cudaEventDestroy(x);
+    for (auto &e : h->evK)
+        for (auto &x : e)
+            if (x) cudaEventDestroy(x);
+}
+
 int setup(pbc_jk *h, const pbc_cell *cell, const pbc_atoms *atoms, const pbc_shells *shells, double omega)
 {
     const pbc_cutoffs &cut = h->cut;
@@ -203,6 +221,7 @@ int setup(pbc_jk *h, const pbc_cell *cell, const pbc_atoms *atoms, const pbc_she
         if (shells->nprim[s] < 1) return fail(h, PBC_JK_ERR_INVALID_ARG, "shell without primitives");
         if (shells->atom[s] < 0 || shells->atom[s] >= natom) return fail(h, PBC_JK_ERR_INVALID_ARG, "shell atom index out of range");
         sh_l[s] = l; sh_ao[s] = nbf; sh_atom[s] = shells->atom[s];
+        h->has_l[l] = true;
         nbf += ncart(l);
         scx[s] = atoms->xyz[3 * sh_atom[s]]; scy[s] = atoms->xyz[3 * sh_atom[s] + 1]; scz[s] = atoms->xyz[3 * sh_atom[s] + 2];
         for (int k = 0; k < shells->nprim[s]; ++k) {
@@ -529,6 +548,8 @@ int setup(pbc_jk *h, const pbc_cell *cell, const pbc_atoms *atoms, const pbc_she
         CK(pool.alloc(&h->rho, (size_t)2 * nb));
         CK(pool.alloc(&h->hostP, N * N)); CK(pool.alloc(&h->hostJ, N * N)); CK(pool.alloc(&h->hostK, N * N));
         for (auto &e : h->ev) CK(cudaEventCreate(&e));
+        for (auto &e : h->evJ) { CK(cudaEventCreate(&e[0])); CK(cudaEventCreate(&e[1])); }
+        for (auto &e : h->evK) { CK(cudaEventCreate(&e[0])); CK(cudaEventCreate(&e[1])); }
     }
     // ---- A3: overlap S = rho_mn(G = 0) (eq 21) ----
     {
@@ -575,8 +596,7 @@ int pbc_jk_create(const pbc_cell *cell, const pbc_atoms *atoms, const pbc_shells
     if (rc != PBC_JK_OK) {
         g_create_error = h->err;
         h->pool.free_all();
-        for (auto &e : h->ev)
-            if (e) cudaEventDestroy(e);
+        destroy_events(h);
         delete h;
         return rc;
     }
@@ -611,6 +631,10 @@ int pbc_jk_build(pbc_jk *h, const double *P, double *J, double *K, void *cuda_st
     const bool doSR = h->parts & 1, doLR = h->parts & 2, doSELF = h->parts & 4;
     CK(cudaMemsetAsync(h->counters, 0, CNT_N * 8, st));
     CK(cudaEventRecord(h->ev[0], st));
+    int64_t nl = 0;                      // kernels launched by this build
+    for (auto &b : h->ranJ) b = false;
+    for (auto &b : h->ranK) b = false;
+    nl += 2;
     launch_scale_density(P, h->Pp, N, Np, h->fcomp, h->maxbits, h->lnPmax, st);
     SRParams sp;
     sp.K = h->K; sp.U = h->U; sp.KJ = h->KJ; sp.lat = h->lat; sp.sh = h->sh;
@@ -619,15 +643,29 @@ int pbc_jk_build(pbc_jk *h, const double *P, double *J, double *K, void *cuda_st
     sp.ln_tau = std::log(h->cut.d_schwarz > 0 ? h->cut.d_schwarz : 1e-13);
     sp.rcut2 = h->cut.r_cut > 0 ? h->cut.r_cut * h->cut.r_cut : std::numeric_limits<double>::infinity();
     sp.counters = h->counters;
-    if (J && doSR) launch_hermite_density(h->U, h->sh, h->KJ, h->Pp, Np, h->Dt, st);
+    if (J && doSR && h->KJ.n > 0) {
+        launch_hermite_density(h->U, h->sh, h->KJ, h->Pp, Np, h->Dt, st);
+        ++nl;
+    }
     CK(cudaEventRecord(h->ev[1], st));
     // ---- A5: real-space J ----
     if (J && doSR) {
         CK(cudaMemsetAsync(h->Jt, 0, (size_t)nherm(4) * std::max(h->U.n, 1) * 8, st));
         CK(cudaMemsetAsync(h->Jsr, 0, NN * 8, st));
         for (int LB = 0; LB <= 4; ++LB)
-            for (int LK = 0; LK <= 4; ++LK) launch_sr_j(LB, LK, sp, h->jbra[LB], h->njbra[LB], st);
-        launch_j_backtransform(h->U, h->sh, h->Jt, h->Jsr, N, st);
+            for (int LK = 0; LK <= 4; ++LK) {
+                if (h->njbra[LB] <= 0 || h->njbra[LK] <= 0) continue;
+                const int cls = LB * 5 + LK;
+                if (h->profile) CK(cudaEventRecord(h->evJ[cls][0], st));
+                launch_sr_j(LB, LK, sp, h->jbra[LB], h->njbra[LB], st);
+                if (h->profile) CK(cudaEventRecord(h->evJ[cls][1], st));
+                h->ranJ[cls] = true;
+                ++nl;
+            }
+        if (h->U.nsp > 0) {
+            launch_j_backtransform(h->U, h->sh, h->Jt, h->Jsr, N, st);
+            ++nl;
+        }
     }
     CK(cudaEventRecord(h->ev[2], st));
     // ---- A6: real-space K ----
@@ -636,8 +674,15 @@ int pbc_jk_build(pbc_jk *h, const double *P, double *J, double *K, void *cuda_st
         for (int la = LMAX; la >= 0; --la)
             for (int ld = la; ld >= 0; --ld)
                 for (int lb = LMAX; lb >= 0; --lb)
-                    for (int lc = LMAX; lc >= 0; --lc)
+                    for (int lc = LMAX; lc >= 0; --lc) {
+                        if (h->nkblk[la][ld] <= 0 || !h->has_l[lb] || !h->has_l[lc]) continue;
+                        const int cls = ((la * 3 + lb) * 3 + lc) * 3 + ld;
+                        if (h->profile) CK(cudaEventRecord(h->evK[cls][0], st));
                         launch_sr_k(la, lb, lc, ld, sp, h->kblk[la][ld], h->nkblk[la][ld], st);
+                        if (h->profile) CK(cudaEventRecord(h->evK[cls][1], st));
+                        h->ranK[cls] = true;
+                        ++nl;
+                    }
     }
     CK(cudaEventRecord(h->ev[3], st));
     // ---- A7/A8: reciprocal space, batches of G ----
@@ -649,6 +694,7 @@ int pbc_jk_build(pbc_jk *h, const double *P, double *J, double *K, void *cuda_st
         for (int g0 = 0; g0 < h->nG; g0 += h->nb) {
             const int nb = std::min(h->nb, h->nG - g0), nslot = 2 * nb;
             launch_agen(h->lr, g0, nb, 0.0, h->Astack, h->ld, st);
+            nl += 1 + (J ? 2 : 0) + (K ? 2 : 0);
             if (J) {
                 launch_rho_reduce(h->Pp, h->Astack, h->ld, Np, N, nslot, h->rho, st);
                 launch_jlr_accum(h->Astack, h->ld, Np, N, nslot, h->rho, 1.0, h->Jlr, st);
@@ -665,6 +711,7 @@ int pbc_jk_build(pbc_jk *h, const double *P, double *J, double *K, void *cuda_st
     // ---- A9: the G = 0 slot, weight -pi/(Omega w^2), A = S ----
     if (doSELF) {
         launch_agen(h->lr, -1, 1, std::sqrt(h->c0), h->Astack, h->ld, st);
+        nl += 1 + (J ? 2 : 0) + (K ? 2 : 0);
         if (J) {
             launch_rho_reduce(h->Pp, h->Astack, h->ld, Np, N, 1, h->rho, st);
             launch_jlr_accum(h->Astack, h->ld, Np, N, 1, h->rho, -1.0, h->Jlr, st);
@@ -680,8 +727,10 @@ int pbc_jk_build(pbc_jk *h, const double *P, double *J, double *K, void *cuda_st
     if (K)
         launch_finalize_k(doSR ? h->Ksr : nullptr, h->sh, needKlr ? h->Klr : nullptr, h->nsplit, strideK, Np, N, h->fcomp,
                           h->shell_of_ao, K, st);
+    nl += (J ? 1 : 0) + (K ? 1 : 0);
     CK(cudaEventRecord(h->ev[5], st));
     CK(cudaGetLastError());
+    h->n_launches = nl;
     h->last_stream = st;
     h->built = true;
     return PBC_JK_OK;
@@ -712,14 +761,59 @@ int pbc_jk_get_stats(pbc_jk *h, pbc_jk_stats_t *out)
         CK(cudaEventSynchronize(h->ev[5]));
         unsigned long long c[CNT_N];
         CK(cudaMemcpy(c, h->counters, sizeof(c), cudaMemcpyDeviceToHost));
-        out->candidates_j = (int64_t)c[CNT_CAND_J]; out->quartets_j = (int64_t)c[CNT_Q_J];
-        out->candidates_k = (int64_t)c[CNT_CAND_K]; out->quartets_k = (int64_t)c[CNT_Q_K];
+        for (int i = 0; i < NCLS_J; ++i) { out->candidates_j += (int64_t)c[CNT_CAND_J + i]; out->quartets_j += (int64_t)c[CNT_Q_J + i]; }
+        for (int i = 0; i < NCLS_K; ++i) { out->candidates_k += (int64_t)c[CNT_CAND_K + i]; out->quartets_k += (int64_t)c[CNT_Q_K + i]; }
+        out->n_launches = h->n_launches;
         float ms[5];
         for (int i = 0; i < 5; ++i) CK(cudaEventElapsedTime(&ms[i], h->ev[i], h->ev[i + 1]));
         float tot;
         CK(cudaEventElapsedTime(&tot, h->ev[0], h->ev[5]));
         out->ms_density = ms[0]; out->ms_sr_j = ms[1]; out->ms_sr_k = ms[2]; out->ms_lr = ms[3] + ms[4]; out->ms_total = tot;
     }
+    return PBC_JK_OK;
+}
+
+int pbc_jk_set_profile(pbc_jk *h, int32_t on)
+{
+    if (!h) return PBC_JK_ERR_INVALID_ARG;
+    h->profile = on != 0;
+    return PBC_JK_OK;
+}
+
+int pbc_jk_get_class_stats(pbc_jk *h, pbc_jk_class_stat *out, int32_t cap, int32_t *n_out)
+{
+    if (!h || !n_out || (cap > 0 && !out)) return PBC_JK_ERR_INVALID_ARG;
+    *n_out = 0;
+    if (!h->built) return PBC_JK_OK;
+    CK(cudaEventSynchronize(h->ev[5]));
+    unsigned long long c[CNT_N];
+    CK(cudaMemcpy(c, h->counters, sizeof(c), cudaMemcpyDeviceToHost));
+    int n = 0;
+    for (int cls = 0; cls < NCLS_J; ++cls) {
+        if (!h->ranJ[cls]) continue;
+        if (n < cap) {
+            pbc_jk_class_stat &s = out[n];
+            s.kind = 0; s.l[0] = cls / 5; s.l[1] = cls % 5; s.l[2] = s.l[3] = 0;
+            s.quartets = (int64_t)c[CNT_Q_J + cls]; s.candidates = (int64_t)c[CNT_CAND_J + cls];
+            float ms = 0.f;
+            if (h->profile) CK(cudaEventElapsedTime(&ms, h->evJ[cls][0], h->evJ[cls][1]));
+            s.ms = ms;
+        }
+        ++n;
+    }
+    for (int cls = 0; cls < NCLS_K; ++cls) {
+        if (!h->ranK[cls]) continue;
+        if (n < cap) {
+            pbc_jk_class_stat &s = out[n];
+            s.kind = 1; s.l[0] = cls / 27; s.l[1] = (cls / 9) % 3; s.l[2] = (cls / 3) % 3; s.l[3] = cls % 3;
+            s.quartets = (int64_t)c[CNT_Q_K + cls]; s.candidates = (int64_t)c[CNT_CAND_K + cls];
+            float ms = 0.f;
+            if (h->profile) CK(cudaEventElapsedTime(&ms, h->evK[cls][0], h->evK[cls][1]));
+            s.ms = ms;
+        }
+        ++n;
+    }
+    *n_out = n;
     return PBC_JK_OK;
 }
 
@@ -730,8 +824,7 @@ int pbc_jk_destroy(pbc_jk *h)
     if (!h) return PBC_JK_OK;
     cudaDeviceSynchronize();
     h->pool.free_all();
-    for (auto &e : h->ev)
-        if (e) cudaEventDestroy(e);
+    destroy_events(h);
     delete h;
     return PBC_JK_OK;
 }

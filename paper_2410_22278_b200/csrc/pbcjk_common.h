@@ -76,7 +76,10 @@ struct ShellInfo {
     int nshell, nbf;
 };
 
-// counters (device, int64): 0 cand_j, 1 quart_j, 2 cand_k, 3 quart_k
-enum { CNT_CAND_J = 0, CNT_Q_J = 1, CNT_CAND_K = 2, CNT_Q_K = 3, CNT_N = 8 };
+// counters (device, int64), one slot per kernel class:
+//   J class index = LB*5 + LK (Hermite orders of bra and ket), K class index = ((la*3+lb)*3+lc)*3+ld
+constexpr int NCLS_J = 25, NCLS_K = 81;
+enum { CNT_CAND_J = 0, CNT_Q_J = NCLS_J, CNT_CAND_K = 2 * NCLS_J, CNT_Q_K = 2 * NCLS_J + NCLS_K,
+       CNT_N = 2 * NCLS_J + 2 * NCLS_K };
 
 }  // namespace pbcjk

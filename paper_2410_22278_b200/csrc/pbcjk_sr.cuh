@@ -213,8 +213,8 @@ __global__ void __launch_bounds__(128) sr_j_kernel(SRParams p, const int *__rest
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) c += __shfl_xor_sync(0xffffffffu, c, o);
     if (lane == 0) {
-        atomicAdd(p.counters + CNT_CAND_J, c);
-        atomicAdd(p.counters + CNT_Q_J, e32 + (unsigned long long)qn);
+        atomicAdd(p.counters + CNT_CAND_J + LB * 5 + LK, c);
+        atomicAdd(p.counters + CNT_Q_J + LB * 5 + LK, e32 + (unsigned long long)qn);
     }
 }
 
@@ -417,8 +417,9 @@ __global__ void __launch_bounds__(KWARPS * 32) sr_k_kernel(SRParams p, const int
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) c += __shfl_xor_sync(0xffffffffu, c, o);
     if (lane == 0) {
-        atomicAdd(p.counters + CNT_CAND_K, c);
-        atomicAdd(p.counters + CNT_Q_K, (unsigned long long)nq * 32ull + nflush);
+        constexpr int cls = ((LA * 3 + LB) * 3 + LC) * 3 + LD;
+        atomicAdd(p.counters + CNT_CAND_K + cls, c);
+        atomicAdd(p.counters + CNT_Q_K + cls, (unsigned long long)nq * 32ull + nflush);
     }
 }
 
