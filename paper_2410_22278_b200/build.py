@@ -24,7 +24,11 @@ INCLUDE = os.path.join(os.path.dirname(HERE), "include")
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC,-fopenmp,-O2", "-I", INCLUDE]
 
-HEADERS = ["pbcjk_common.h", "pbcjk_md.cuh", "pbcjk_sr.cuh", "pbcjk_lr.cuh", os.path.join(INCLUDE, "pbc_jk.h")]
+# headers each source includes (directly or not): a change recompiles only the units that see it
+_SR_H = ["pbcjk_common.h", "pbcjk_md.cuh", "pbcjk_sr.cuh"]
+HEADERS = {"pbcjk_api.cu": _SR_H + ["pbcjk_lr.cuh", os.path.join(INCLUDE, "pbc_jk.h")],
+           "pbcjk_lr.cu": ["pbcjk_common.h", "pbcjk_md.cuh", "pbcjk_lr.cuh"],
+           "sr_dispatch.cu": _SR_H, "sr_j_inst.cu": _SR_H, "sr_k_inst.cu": _SR_H}
 
 
 def _units():
@@ -41,7 +45,7 @@ def _units():
 
 def _digest(src: str, defs) -> str:
     h = hashlib.sha256()
-    for f in [os.path.join(CSRC, src)] + [f if os.path.isabs(f) else os.path.join(CSRC, f) for f in HEADERS]:
+    for f in [os.path.join(CSRC, src)] + [f if os.path.isabs(f) else os.path.join(CSRC, f) for f in HEADERS[src]]:
         with open(f, "rb") as fh:
             h.update(fh.read())
     # flags enter the key with the checkout path stripped: the objects built here stay valid on the GPU box

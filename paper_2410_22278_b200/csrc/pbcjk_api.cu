@@ -79,6 +79,8 @@ struct pbc_jk {
     double *Pp = nullptr, *lnPmax = nullptr, *Dt = nullptr, *Jt = nullptr, *Jsr = nullptr, *Jlr = nullptr;
     double *Ksr = nullptr, *Klr = nullptr, *Astack = nullptr, *Zstack = nullptr, *rho = nullptr;
     double *hostP = nullptr, *hostJ = nullptr, *hostK = nullptr;     // device staging of build_host
+    double *LT = nullptr, *chol_d = nullptr, *chol_s = nullptr;      // factor P' = L L^T of the K^LR contraction
+    int *chol_dyn = nullptr;
     unsigned long long *maxbits = nullptr, *counters = nullptr;
     int nb = 1, nsplit = 1;
     bool has_l[LMAX + 1] = {};
@@ -546,6 +548,8 @@ int setup(pbc_jk *h, const pbc_cell *cell, const pbc_atoms *atoms, const pbc_she
         CK(pool.alloc(&h->Astack, Np * h->ld)); CK(cudaMemset(h->Astack, 0, Np * h->ld * 8));
         CK(pool.alloc(&h->Zstack, Np * h->ld));
         CK(pool.alloc(&h->rho, (size_t)2 * nb));
+        CK(pool.alloc(&h->LT, Np * Np)); CK(pool.alloc(&h->chol_d, 2 * Np)); CK(pool.alloc(&h->chol_s, 2));
+        CK(pool.alloc(&h->chol_dyn, 4));
         CK(pool.alloc(&h->hostP, N * N)); CK(pool.alloc(&h->hostJ, N * N)); CK(pool.alloc(&h->hostK, N * N));
         for (auto &e : h->ev) CK(cudaEventCreate(&e));
         for (auto &e : h->evJ) { CK(cudaEventCreate(&e[0])); CK(cudaEventCreate(&e[1])); }
@@ -690,6 +694,23 @@ int pbc_jk_build(pbc_jk *h, const double *P, double *J, double *K, void *cuda_st
     if (needJlr) CK(cudaMemsetAsync(h->Jlr, 0, NN * 8, st));
     if (needKlr) CK(cudaMemsetAsync(h->Klr, 0, (size_t)h->nsplit * Np * Np * 8, st));
     const size_t strideK = (size_t)Np * Np;
+    // K^LR = sum_slots Y^T Y with Y = L^T A', P' = L L^T (device-side rank; dense fallback inside the same kernels)
+    if (needKlr) {
+        launch_factor_density(h->Pp, N, Np, h->LT, h->chol_d, h->chol_dyn, h->chol_s, h->Zstack, st);
+        nl += factor_density_launches(N);
+    }
+    auto klr_batch = [&](int nslot, double alpha, int nsplit) {
+        GemmArgs g1;                                     // Y = L^T [A'_1 A'_2 ...]  (rows >= rank skipped)
+        g1.M = Np; g1.Nc = nslot * Np; g1.Kb = Np; g1.nbatch = 1; g1.A = h->LT; g1.lda = Np; g1.B = h->Astack; g1.ldb = h->ld;
+        g1.C = h->Zstack; g1.ldc = h->ld; g1.dyn = h->chol_dyn; g1.use_dyn = 1;
+        launch_dgemm(g1, st);
+        GemmArgs g2;                                     // K += alpha sum_slot Y_slot^T Y_slot  (lower tiles)
+        g2.M = Np; g2.Nc = Np; g2.Kb = Np; g2.nbatch = nslot; g2.alpha = alpha; g2.transA = true;
+        g2.A = h->Zstack; g2.lda = h->ld; g2.strideA = Np; g2.B = h->Zstack; g2.ldb = h->ld; g2.strideB = Np;
+        g2.B_alt = h->Astack; g2.beta = 1.0; g2.C = h->Klr; g2.ldc = Np; g2.strideC = strideK; g2.nsplit = nsplit;
+        g2.dyn = h->chol_dyn; g2.use_dyn = 2 | 4; g2.lower_only = 1;
+        launch_dgemm(g2, st);
+    };
     if (doLR) {
         for (int g0 = 0; g0 < h->nG; g0 += h->nb) {
             const int nb = std::min(h->nb, h->nG - g0), nslot = 2 * nb;
@@ -699,13 +720,7 @@ int pbc_jk_build(pbc_jk *h, const double *P, double *J, double *K, void *cuda_st
                 launch_rho_reduce(h->Pp, h->Astack, h->ld, Np, N, nslot, h->rho, st);
                 launch_jlr_accum(h->Astack, h->ld, Np, N, nslot, h->rho, 1.0, h->Jlr, st);
             }
-            if (K) {
-                // Z = P' [A'_1 A'_2 ...]
-                launch_dgemm(Np, nslot * Np, Np, 1, 1.0, h->Pp, Np, 0, h->Astack, h->ld, 0, 0.0, h->Zstack, h->ld, 0, 1, st);
-                // K += sum_slot A'_slot Z_slot
-                launch_dgemm(Np, Np, Np, nslot, 1.0, h->Astack, h->ld, Np, h->Zstack, h->ld, Np, 1.0, h->Klr, Np, strideK,
-                             std::min(h->nsplit, nslot), st);
-            }
+            if (K) klr_batch(nslot, 1.0, std::min(h->nsplit, nslot));
         }
     }
     // ---- A9: the G = 0 slot, weight -pi/(Omega w^2), A = S ----
@@ -716,10 +731,7 @@ int pbc_jk_build(pbc_jk *h, const double *P, double *J, double *K, void *cuda_st
             launch_rho_reduce(h->Pp, h->Astack, h->ld, Np, N, 1, h->rho, st);
             launch_jlr_accum(h->Astack, h->ld, Np, N, 1, h->rho, -1.0, h->Jlr, st);
         }
-        if (K) {
-            launch_dgemm(Np, Np, Np, 1, 1.0, h->Pp, Np, 0, h->Astack, h->ld, 0, 0.0, h->Zstack, h->ld, 0, 1, st);
-            launch_dgemm(Np, Np, Np, 1, -1.0, h->Astack, h->ld, 0, h->Zstack, h->ld, 0, 1.0, h->Klr, Np, strideK, 1, st);
-        }
+        if (K) klr_batch(1, -1.0, 1);
     }
     CK(cudaEventRecord(h->ev[4], st));
     // ---- A10 ----

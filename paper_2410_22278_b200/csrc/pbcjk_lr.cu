@@ -283,7 +283,6 @@ namespace {
 constexpr int BM = 128, BN = 128, BK = 16;
 constexpr int SA = BK + 4;    // row stride of the A tile [m][k]: (lane/4)*20 + lane%4 hits every bank pair twice
 constexpr int SB = BN + 8;    // row stride of the B tile [k][n]: (lane%4)*136 + lane/4 likewise
-constexpr int GEMM_SMEM = 2 * (BM * SA + BK * SB) * (int)sizeof(double);
 
 __device__ __forceinline__ void cp_async16(void *smem, const void *gmem)
 {
@@ -298,16 +297,33 @@ __device__ __forceinline__ void dmma(double &c0, double &c1, double a, double b)
 }
 }  // namespace
 
+// C[z] = beta*C[z] + alpha * sum_{b in batches(z)} op(A_b) B_b
+//   TA = false: A_b is row-major M x Kb (k contiguous);  TA = true: A_b is stored as Kb x M (m contiguous),
+//   i.e. op(A) = A^T -- the Y^T Y form of the reciprocal-space K contraction.
+//   dyn (device, may be null): dyn[0] = rank r of the factor P' = L L^T (or N in the fallback), dyn[1] = use B_alt.
+//   use_dyn bit 0: only row tiles with bm*BM < r are computed; bit 1: Kb = roundup16(r); bit 2: B = B_alt if dyn[1];
+//   lower_only: tiles with bn > bm are skipped (symmetric result, completed in finalise).
+template <bool TA>
 __global__ void __launch_bounds__(256) dgemm_kernel(int Kb, int nbatch, double alpha, const double *__restrict__ A, size_t lda,
                                                     size_t strideA, const double *__restrict__ B, size_t ldb, size_t strideB,
-                                                    double beta, double *__restrict__ C, size_t ldc, size_t strideC, int nsplit)
+                                                    double beta, double *__restrict__ C, size_t ldc, size_t strideC, int nsplit,
+                                                    const int *__restrict__ dyn, int use_dyn, const double *__restrict__ B_alt,
+                                                    int lower_only)
 {
     extern __shared__ __align__(16) double smem[];
-    double *As = smem;                       // [2][BM*SA]
-    double *Bs = smem + 2 * BM * SA;         // [2][BK*SB]
+    constexpr int A_TILE = TA ? BK * SB : BM * SA;
+    double *As = smem;                       // [2][A_TILE]
+    double *Bs = smem + 2 * A_TILE;          // [2][BK*SB]
     const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
     const int wm = w >> 2, wn = w & 3;
     const int bm = blockIdx.y, bn = blockIdx.x, z = blockIdx.z;
+    if (lower_only && bn > bm) return;
+    if (dyn) {
+        const int r = dyn[0];
+        if ((use_dyn & 1) && bm * BM >= r) return;
+        if (use_dyn & 2) Kb = ((r + BK - 1) / BK) * BK;
+        if ((use_dyn & 4) && dyn[1]) B = B_alt;
+    }
     const int bat0 = (int)((long long)nbatch * z / nsplit), bat1 = (int)((long long)nbatch * (z + 1) / nsplit);
     const int kt_per = Kb / BK;
     const int ntile = (bat1 - bat0) * kt_per;
@@ -321,13 +337,22 @@ __global__ void __launch_bounds__(256) dgemm_kernel(int Kb, int nbatch, double a
 
     auto load_tile = [&](int t, int buf) {
         const int b = bat0 + t / kt_per, k0 = (t % kt_per) * BK;
-        const double *Ab = A + (size_t)b * strideA + (size_t)(bm * BM) * lda + k0;
         const double *Bb = B + (size_t)b * strideB + (size_t)k0 * ldb + bn * BN;
-        double *as = As + buf * BM * SA, *bs = Bs + buf * BK * SB;
+        double *as = As + buf * A_TILE, *bs = Bs + buf * BK * SB;
+        if (TA) {
+            const double *Ab = A + (size_t)b * strideA + (size_t)k0 * lda + bm * BM;
 #pragma unroll
-        for (int c = tid; c < BM * BK / 2; c += 256) {
-            const int row = c >> 3, c2 = c & 7;
-            cp_async16(as + row * SA + c2 * 2, Ab + (size_t)row * lda + c2 * 2);
+            for (int c = tid; c < BK * BM / 2; c += 256) {
+                const int row = c >> 6, c2 = c & 63;
+                cp_async16(as + row * SB + c2 * 2, Ab + (size_t)row * lda + c2 * 2);
+            }
+        } else {
+            const double *Ab = A + (size_t)b * strideA + (size_t)(bm * BM) * lda + k0;
+#pragma unroll
+            for (int c = tid; c < BM * BK / 2; c += 256) {
+                const int row = c >> 3, c2 = c & 7;
+                cp_async16(as + row * SA + c2 * 2, Ab + (size_t)row * lda + c2 * 2);
+            }
         }
 #pragma unroll
         for (int c = tid; c < BK * BN / 2; c += 256) {
@@ -347,13 +372,14 @@ __global__ void __launch_bounds__(256) dgemm_kernel(int Kb, int nbatch, double a
             asm volatile("cp.async.wait_group 0;\n" ::);
         }
         __syncthreads();
-        const double *as = As + buf * BM * SA + (wm * 64 + (lane >> 2)) * SA + (lane & 3);
+        const double *as = TA ? As + buf * A_TILE + (lane & 3) * SB + wm * 64 + (lane >> 2)
+                              : As + buf * A_TILE + (wm * 64 + (lane >> 2)) * SA + (lane & 3);
         const double *bs = Bs + buf * BK * SB + (lane & 3) * SB + wn * 32 + (lane >> 2);
 #pragma unroll
         for (int kk = 0; kk < BK; kk += 4) {
             double a[8], b[4];
 #pragma unroll
-            for (int i = 0; i < 8; ++i) a[i] = as[i * 8 * SA + kk];
+            for (int i = 0; i < 8; ++i) a[i] = TA ? as[kk * SB + i * 8] : as[i * 8 * SA + kk];
 #pragma unroll
             for (int j = 0; j < 4; ++j) b[j] = bs[kk * SB + j * 8];
 #pragma unroll
@@ -380,19 +406,148 @@ __global__ void __launch_bounds__(256) dgemm_kernel(int Kb, int nbatch, double a
         }
 }
 
-void launch_dgemm(int M, int Nc, int Kb, int nbatch, double alpha, const double *A, size_t lda, size_t strideA,
-                  const double *B, size_t ldb, size_t strideB, double beta, double *C, size_t ldc, size_t strideC,
-                  int nsplit, cudaStream_t st)
+void launch_dgemm(const GemmArgs &g, cudaStream_t st)
 {
     static bool attr_set = false;
+    constexpr int smemN = 2 * (BM * SA + BK * SB) * (int)sizeof(double), smemT = 2 * (2 * BK * SB) * (int)sizeof(double);
     if (!attr_set) {
-        cudaFuncSetAttribute(dgemm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, GEMM_SMEM);
+        cudaFuncSetAttribute(dgemm_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smemN);
+        cudaFuncSetAttribute(dgemm_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smemT);
         attr_set = true;
     }
-    dim3 grid(Nc / BN, M / BM, nsplit);
-    dgemm_kernel<<<grid, 256, GEMM_SMEM, st>>>(Kb, nbatch, alpha, A, lda, strideA, B, ldb, strideB, beta, C, ldc, strideC,
-                                               nsplit);
+    dim3 grid(g.Nc / BN, g.M / BM, g.nsplit);
+    if (g.transA)
+        dgemm_kernel<true><<<grid, 256, smemT, st>>>(g.Kb, g.nbatch, g.alpha, g.A, g.lda, g.strideA, g.B, g.ldb, g.strideB, g.beta,
+                                                     g.C, g.ldc, g.strideC, g.nsplit, g.dyn, g.use_dyn, g.B_alt, g.lower_only);
+    else
+        dgemm_kernel<false><<<grid, 256, smemN, st>>>(g.Kb, g.nbatch, g.alpha, g.A, g.lda, g.strideA, g.B, g.ldb, g.strideB, g.beta,
+                                                      g.C, g.ldc, g.strideC, g.nsplit, g.dyn, g.use_dyn, g.B_alt, g.lower_only);
 }
+
+// ---------------------------------------------------------------- factor of P' for the K contraction (A8)
+// K^LR = sum_G w Re[conj(A) P' A] costs 8 N^3 flop per G with a dense P'.  SCF densities are P = C C^T of rank
+// n_occ << N, so P' = L L^T is factored once per build by a diagonally pivoted Cholesky decomposition (stop at
+// residual diagonal <= 1e-13 max diag) and K^LR = sum_slots Y^T Y with Y = L^T A' (8 r N^2 flop per G).  A P' that is
+// not positive semidefinite fails the residual test |P' - L L^T| and falls back, on the device, to L = P', r = N,
+// K^LR = sum (P'A')^T A' -- same kernels, no host round trip.
+//   dyn[0] = rank, dyn[1] = fallback flag, dyn[2] = done;  dscal[0] = max diag, dscal[1] = max |residual| (bits)
+__global__ void chol_init_kernel(const double *__restrict__ Pp, int N, int Np, double *__restrict__ d0, int *dyn,
+                                 double *dscal)
+{
+    __shared__ double s[32];
+    double m = 0.0;
+    for (int i = threadIdx.x; i < N; i += blockDim.x) {
+        const double v = Pp[(size_t)i * Np + i];
+        d0[i] = v;
+        m = fmax(m, v);
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) m = fmax(m, __shfl_xor_sync(0xffffffffu, m, o));
+    if ((threadIdx.x & 31) == 0) s[threadIdx.x >> 5] = m;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        for (int w = 1; w < (int)(blockDim.x >> 5); ++w) m = fmax(m, s[w]);
+        dscal[0] = m;
+        dscal[1] = 0.0;
+        dyn[0] = 0; dyn[1] = 0; dyn[2] = 0;
+    }
+}
+
+// step k: every block finds the pivot (largest residual diagonal, lowest index on ties) on its own, then forms its
+// rows of column k.  d_in / d_out alternate between steps so no block reads what another writes.
+__global__ void __launch_bounds__(128) chol_step_kernel(int k, const double *__restrict__ Pp, int N, int Np,
+                                                        double *__restrict__ LT, const double *__restrict__ d_in,
+                                                        double *__restrict__ d_out, int *dyn, const double *__restrict__ dscal)
+{
+    if (dyn[2]) return;
+    __shared__ double sv[4];
+    __shared__ int si[4];
+    double best = -1.0;
+    int bi = 0x7fffffff;
+    for (int i = threadIdx.x; i < N; i += 128) {
+        const double v = d_in[i];
+        if (v > best) { best = v; bi = i; }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        const double ov = __shfl_xor_sync(0xffffffffu, best, o);
+        const int oi = __shfl_xor_sync(0xffffffffu, bi, o);
+        if (ov > best || (ov == best && oi < bi)) { best = ov; bi = oi; }
+    }
+    if ((threadIdx.x & 31) == 0) { sv[threadIdx.x >> 5] = best; si[threadIdx.x >> 5] = bi; }
+    __syncthreads();
+    best = sv[0]; bi = si[0];
+#pragma unroll
+    for (int w = 1; w < 4; ++w)
+        if (sv[w] > best || (sv[w] == best && si[w] < bi)) { best = sv[w]; bi = si[w]; }
+    if (!(best > 1e-13 * dscal[0]) || !(best > 0.0)) {
+        if (blockIdx.x == 0 && threadIdx.x == 0) dyn[2] = 1;
+        return;
+    }
+    const int i = blockIdx.x * 128 + threadIdx.x;
+    if (i < N) {
+        double s0 = Pp[(size_t)bi * Np + i], s1 = 0.0, s2 = 0.0, s3 = 0.0;
+        int j = 0;
+        for (; j + 4 <= k; j += 4) {
+            s0 = fma(-LT[(size_t)j * Np + i], LT[(size_t)j * Np + bi], s0);
+            s1 = fma(-LT[(size_t)(j + 1) * Np + i], LT[(size_t)(j + 1) * Np + bi], s1);
+            s2 = fma(-LT[(size_t)(j + 2) * Np + i], LT[(size_t)(j + 2) * Np + bi], s2);
+            s3 = fma(-LT[(size_t)(j + 3) * Np + i], LT[(size_t)(j + 3) * Np + bi], s3);
+        }
+        for (; j < k; ++j) s0 = fma(-LT[(size_t)j * Np + i], LT[(size_t)j * Np + bi], s0);
+        const double root = sqrt(best);
+        double v = ((s0 + s1) + (s2 + s3)) / root;
+        if (i == bi) v = root;
+        LT[(size_t)k * Np + i] = v;
+        d_out[i] = (i == bi) ? 0.0 : d_in[i] - v * v;
+    }
+    if (blockIdx.x == 0 && threadIdx.x == 0) dyn[0] = k + 1;
+}
+
+// max |P' - L L^T| over the lower-triangular tiles (R holds L L^T there)
+__global__ void chol_residual_kernel(const double *__restrict__ Pp, const double *__restrict__ R, int N, int Np,
+                                     unsigned long long *resbits)
+{
+    const int n = blockIdx.x * blockDim.x + threadIdx.x, m = blockIdx.y;
+    double v = 0.0;
+    if (n < N && (n / BN) <= (m / BM)) v = fabs(Pp[(size_t)m * Np + n] - R[(size_t)m * Np + n]);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, o));
+    if ((threadIdx.x & 31) == 0 && v > 0.0) atomicMax(resbits, (unsigned long long)__double_as_longlong(v));
+}
+
+// not positive semidefinite (or badly conditioned): L := P', r := N, stage-2 B operand := A'
+__global__ void chol_fallback_kernel(const double *__restrict__ Pp, int N, int Np, double *__restrict__ LT, int *dyn,
+                                     const double *__restrict__ dscal)
+{
+    const double res = __longlong_as_double((long long)((const unsigned long long *)dscal)[1]);
+    if (res <= 1e-12 * fmax(dscal[0], 1e-300)) return;
+    const size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx < (size_t)Np * Np) LT[idx] = Pp[idx];
+    if (idx == 0) { dyn[0] = N; dyn[1] = 1; }
+}
+
+void launch_factor_density(const double *Pp, int N, int Np, double *LT, double *dbuf, int *dyn, double *dscal, double *scratch,
+                           cudaStream_t st)
+{
+    cudaMemsetAsync(LT, 0, (size_t)Np * Np * sizeof(double), st);
+    chol_init_kernel<<<1, 1024, 0, st>>>(Pp, N, Np, dbuf, dyn, dscal);
+    const int nblk = (N + 127) / 128;
+    for (int k = 0; k < N; ++k)
+        chol_step_kernel<<<nblk, 128, 0, st>>>(k, Pp, N, Np, LT, dbuf + (size_t)(k & 1) * Np, dbuf + (size_t)((k + 1) & 1) * Np, dyn,
+                                               dscal);
+    // residual: scratch = L L^T on the lower-triangular tiles
+    GemmArgs g;
+    g.M = Np; g.Nc = Np; g.Kb = Np; g.nbatch = 1; g.alpha = 1.0; g.A = LT; g.lda = Np; g.strideA = 0; g.B = LT; g.ldb = Np;
+    g.strideB = 0; g.beta = 0.0; g.C = scratch; g.ldc = Np; g.strideC = 0; g.nsplit = 1; g.transA = true; g.dyn = dyn;
+    g.use_dyn = 2; g.lower_only = 1;
+    launch_dgemm(g, st);
+    dim3 grid((N + 127) / 128, N);
+    chol_residual_kernel<<<grid, 128, 0, st>>>(Pp, scratch, N, Np, (unsigned long long *)(dscal + 1));
+    const size_t tot = (size_t)Np * Np;
+    chol_fallback_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, st>>>(Pp, N, Np, LT, dyn, dscal);
+}
+int factor_density_launches(int N) { return 1 + N + 3; }
 
 // ---------------------------------------------------------------- finalise (A10)
 __global__ void finalize_j_kernel(const double *__restrict__ Jsr, const double *__restrict__ Jlr, int N,
@@ -427,10 +582,14 @@ __global__ void finalize_k_kernel(const double *__restrict__ Ksr, ShellInfo sh, 
         else v = Ksr[(size_t)n * N + m];
     }
     if (Klr) {
+        // only the tiles with (row tile >= column tile) were computed (K^LR is symmetric)
+        const int tm = m / 128, tn = n / 128;
         double t = 0.0;
-        for (int z = 0; z < nsplit; ++z)
-            t += Klr[z * strideK + (size_t)m * Np + n] + Klr[z * strideK + (size_t)n * Np + m];
-        v += 0.5 * t;
+        for (int z = 0; z < nsplit; ++z) {
+            const double lo = Klr[z * strideK + (size_t)m * Np + n], up = Klr[z * strideK + (size_t)n * Np + m];
+            t += tm > tn ? lo : (tm < tn ? up : 0.5 * (lo + up));
+        }
+        v += t;
     }
     K[(size_t)m * N + n] = f[m] * f[n] * v;
 }

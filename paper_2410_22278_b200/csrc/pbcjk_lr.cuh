@@ -33,11 +33,28 @@ void launch_rho_reduce(const double *Pp, const double *Astack, size_t ld, int Np
 // Jacc[m][n] += sign * sum_slot A'[slot][m][n] rho'[slot]
 void launch_jlr_accum(const double *Astack, size_t ld, int Np, int N, int nslot, const double *rho, double sign,
                       double *Jacc, cudaStream_t st);
-// C[M x Nc] (ldc) = beta*C + alpha * sum_b A_b[M x Kb](lda) B_b[Kb x Nc](ldb); all dims multiples of
-// 128 (M, Nc) / 16 (Kb); grid.z = nsplit partial results C + z*strideC over disjoint batch ranges.
-void launch_dgemm(int M, int Nc, int Kb, int nbatch, double alpha, const double *A, size_t lda, size_t strideA,
-                  const double *B, size_t ldb, size_t strideB, double beta, double *C, size_t ldc, size_t strideC,
-                  int nsplit, cudaStream_t st);
+// C[z][M x Nc] (ldc) = beta*C + alpha * sum_b op(A_b)[M x Kb] B_b[Kb x Nc](ldb) over the batches of split z;
+// M, Nc multiples of 128, Kb of 16; grid.z = nsplit partial results C + z*strideC over disjoint batch ranges.
+// See dgemm_kernel in pbcjk_lr.cu for transA / dyn / lower_only.
+struct GemmArgs {
+    int M = 0, Nc = 0, Kb = 0, nbatch = 1;
+    double alpha = 1.0;
+    const double *A = nullptr; size_t lda = 0, strideA = 0;
+    const double *B = nullptr; size_t ldb = 0, strideB = 0;
+    double beta = 0.0;
+    double *C = nullptr; size_t ldc = 0, strideC = 0;
+    int nsplit = 1;
+    bool transA = false;
+    const int *dyn = nullptr; int use_dyn = 0;
+    const double *B_alt = nullptr;
+    int lower_only = 0;
+};
+void launch_dgemm(const GemmArgs &g, cudaStream_t st);
+// P' = L L^T (pivoted Cholesky, device-side rank in dyn[0]) with the dense fallback L = P' (dyn[1] = 1);
+// LT: Np x Np (row k = column k of L), dbuf: 2*Np, dyn: 4 ints, dscal: 2 doubles, scratch: Np x Np
+void launch_factor_density(const double *Pp, int N, int Np, double *LT, double *dbuf, int *dyn, double *dscal, double *scratch,
+                           cudaStream_t st);
+int factor_density_launches(int N);
 // out = f f (sum of parts), symmetrised; see pbcjk_lr.cu
 void launch_finalize_j(const double *Jsr, const double *Jlr, int N, const double *fcomp, double *J, cudaStream_t st);
 void launch_finalize_k(const double *Ksr, const ShellInfo &sh, const double *Klr, int nsplit, size_t strideK, int Np,
