@@ -22,13 +22,14 @@ LIB = os.path.join(HERE, "libpbc_jk.so")
 INCLUDE = os.path.join(os.path.dirname(HERE), "include")
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
-              "-Xcompiler", "-fPIC,-fopenmp,-O2", "-I", INCLUDE]
+              "-Xcompiler", "-fPIC,-fopenmp,-O2", "-I", INCLUDE, "-I", OBJ]
 
 # headers each source includes (directly or not): a change recompiles only the units that see it
 _SR_H = ["pbcjk_common.h", "pbcjk_md.cuh", "pbcjk_sr.cuh"]
+_SRK_H = _SR_H + ["pbcjk_srk.cuh", "gen_sr_k.py"]     # the K evaluators are generated into csrc/build/gen
 HEADERS = {"pbcjk_api.cu": _SR_H + ["pbcjk_lr.cuh", os.path.join(INCLUDE, "pbc_jk.h")],
            "pbcjk_lr.cu": ["pbcjk_common.h", "pbcjk_md.cuh", "pbcjk_lr.cuh"],
-           "sr_dispatch.cu": _SR_H, "sr_j_inst.cu": _SR_H, "sr_k_inst.cu": _SR_H}
+           "sr_dispatch.cu": _SR_H, "sr_j_inst.cu": _SR_H, "sr_k_inst.cu": _SRK_H}
 
 
 def _units():
@@ -77,6 +78,10 @@ def _compile(unit, force: bool, verbose: bool) -> str:
 
 def build(force: bool = False, jobs: int = 0, verbose: bool = False) -> str:
     os.makedirs(OBJ, exist_ok=True)
+    sys.path.insert(0, CSRC)
+    import gen_sr_k                                   # straight-line K quartet evaluators, one header per unit
+    sys.path.pop(0)
+    gen_sr_k.main(os.path.join(OBJ, "gen"))
     units = _units()
     jobs = jobs or max(1, min(len(units), (os.cpu_count() or 2)))
     # heaviest units first so the long compiles overlap with everything else

@@ -390,6 +390,31 @@ int setup(pbc_jk *h, const pbc_cell *cell, const pbc_atoms *atoms, const pbc_she
             ipmax[g] = std::max(ipmax[g], kp[i].ip);
         }
         for (int g = 0; g < ns * 3; ++g) off[g + 1] += off[g];
+        // E-product table rows (eq 16-20), filled on the device (etab_kernel)
+        {
+            auto eterms = [](int l1, int l2) {
+                int n = 0;
+                for (int a = 0; a < ncart(l1); ++a)
+                    for (int b = 0; b < ncart(l2); ++b)
+                        n += (cart_x(l1, a) + cart_x(l2, b) + 1) * (cart_y(l1, a) + cart_y(l2, b) + 1) * (cart_z(l1, a) + cart_z(l2, b) + 1);
+                return n;
+            };
+            std::vector<long long> eoff(kp.size());
+            std::vector<int> lA(kp.size()), lB(kp.size());
+            long long tot = 0;
+            for (size_t i = 0; i < kp.size(); ++i) {
+                lA[i] = sh_l[kp[i].shA]; lB[i] = sh_l[kp[i].shB];
+                eoff[i] = tot;
+                tot += eterms(lA[i], lB[i]);
+            }
+            double *etab = nullptr;
+            const int *dlA = nullptr, *dlB = nullptr;
+            CK(pool.upload(&K.eoff, eoff)); CK(pool.alloc(&etab, (size_t)tot));
+            CK(pool.upload(&dlA, lA)); CK(pool.upload(&dlB, lB));
+            K.etab = etab;
+            launch_etab(K, dlA, dlB, etab, 0);
+            CK(cudaGetLastError());
+        }
         CK(pool.upload(&K.aoB, aoB)); CK(pool.upload(&K.off, off));
         CK(pool.upload(&K.ext, ext)); CK(pool.upload(&K.ipmax, ipmax));
         // K block lists per (la >= ld), heaviest first
@@ -533,7 +558,8 @@ int setup(pbc_jk *h, const pbc_cell *cell, const pbc_atoms *atoms, const pbc_she
     // ---- workspaces ----
     {
         const size_t Np = h->Np, N = nbf;
-        int nb = cut.lr_g_batch > 0 ? cut.lr_g_batch : (int)std::min<double>(16.0, std::floor(6.0e9 / (double)(Np * Np * 32)));
+        // G batch: A' and Y stacks of Np x 2nb x Np doubles each, at most 12 GB per stack (180 GB HBM3e per GPU)
+        int nb = cut.lr_g_batch > 0 ? cut.lr_g_batch : (int)std::min<double>(64.0, std::floor(12.0e9 / (double)(Np * Np * 16)));
         nb = std::max(1, std::min(nb, std::max(h->nG, 1)));
         h->nb = nb;
         h->ld = (size_t)2 * nb * Np;
@@ -547,7 +573,7 @@ int setup(pbc_jk *h, const pbc_cell *cell, const pbc_atoms *atoms, const pbc_she
         CK(pool.alloc(&h->Klr, (size_t)h->nsplit * Np * Np));
         CK(pool.alloc(&h->Astack, Np * h->ld)); CK(cudaMemset(h->Astack, 0, Np * h->ld * 8));
         CK(pool.alloc(&h->Zstack, Np * h->ld));
-        CK(pool.alloc(&h->rho, (size_t)2 * nb));
+        CK(pool.alloc(&h->rho, (size_t)rho_scratch_doubles(2 * nb)));
         CK(pool.alloc(&h->LT, Np * Np)); CK(pool.alloc(&h->chol_d, 2 * Np)); CK(pool.alloc(&h->chol_s, 2));
         CK(pool.alloc(&h->chol_dyn, 4));
         CK(pool.alloc(&h->hostP, N * N)); CK(pool.alloc(&h->hostJ, N * N)); CK(pool.alloc(&h->hostK, N * N));
@@ -715,7 +741,7 @@ int pbc_jk_build(pbc_jk *h, const double *P, double *J, double *K, void *cuda_st
         for (int g0 = 0; g0 < h->nG; g0 += h->nb) {
             const int nb = std::min(h->nb, h->nG - g0), nslot = 2 * nb;
             launch_agen(h->lr, g0, nb, 0.0, h->Astack, h->ld, st);
-            nl += 1 + (J ? 2 : 0) + (K ? 2 : 0);
+            nl += 1 + (J ? 3 : 0) + (K ? 2 : 0);
             if (J) {
                 launch_rho_reduce(h->Pp, h->Astack, h->ld, Np, N, nslot, h->rho, st);
                 launch_jlr_accum(h->Astack, h->ld, Np, N, nslot, h->rho, 1.0, h->Jlr, st);
@@ -726,7 +752,7 @@ int pbc_jk_build(pbc_jk *h, const double *P, double *J, double *K, void *cuda_st
     // ---- A9: the G = 0 slot, weight -pi/(Omega w^2), A = S ----
     if (doSELF) {
         launch_agen(h->lr, -1, 1, std::sqrt(h->c0), h->Astack, h->ld, st);
-        nl += 1 + (J ? 2 : 0) + (K ? 2 : 0);
+        nl += 1 + (J ? 3 : 0) + (K ? 2 : 0);
         if (J) {
             launch_rho_reduce(h->Pp, h->Astack, h->ld, Np, N, 1, h->rho, st);
             launch_jlr_accum(h->Astack, h->ld, Np, N, 1, h->rho, -1.0, h->Jlr, st);

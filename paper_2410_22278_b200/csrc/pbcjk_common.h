@@ -36,6 +36,8 @@ struct PairListK {
     const double *Px, *Py, *Pz, *p, *ip, *coef, *lb; // ip = 1/p, lb = ln(bound)
     const double *PAx, *PAy, *PAz, *PBx, *PBy, *PBz; // P - A, P - (B + R2)
     const int *aoB;                                  // AO offset of shell B
+    const double *etab;                              // E^{AB}_t products of every entry (order: gen_sr_k.py)
+    const long long *eoff;                           // [n] row start of entry i in etab
     const int *off;                                  // [nshell*3 + 1]: range of (A, lB)
     const double *ext;                               // [nshell*3]: max |P - A| in the range
     const double *ipmax;                             // [nshell*3]: max 1/p in the range

@@ -94,6 +94,38 @@ void launch_hermite_density(const PairListU &U, const ShellInfo &sh, const KetLi
     hermite_density_kernel<<<(KJ.n + 127) / 128, 128, 0, st>>>(U, sh, KJ, Pp, Np, Dt);
 }
 
+// E^{AB}_t products of every ordered primitive pair-image (eq 16-20), row i at etab[eoff[i]]; order of a row:
+// a in cart(lA), b in cart(lB), tx <= ax+bx, ty <= ay+by, tz <= az+bz (the order gen_sr_k.py assumes).  Runs once
+// per geometry: the K quartet kernels read these rows instead of running the E recursion per quartet.
+__global__ void etab_kernel(PairListK K, const int *__restrict__ lA, const int *__restrict__ lB, double *__restrict__ etab)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= K.n) return;
+    const int la = lA[i], lb = lB[i];
+    const double o2p = 0.5 * K.ip[i];
+    E1Drt ex, ey, ez;
+    ex.build(la, lb, K.PAx[i], K.PBx[i], o2p);
+    ey.build(la, lb, K.PAy[i], K.PBy[i], o2p);
+    ez.build(la, lb, K.PAz[i], K.PBz[i], o2p);
+    double *row = etab + K.eoff[i];
+    const int na = ncart(la), nb = ncart(lb);
+    int n = 0;
+    for (int a = 0; a < na; ++a)
+        for (int b = 0; b < nb; ++b) {
+            int ax, ay, az, bx, by, bz;
+            cart_powers(la, a, ax, ay, az);
+            cart_powers(lb, b, bx, by, bz);
+            for (int tx = 0; tx <= ax + bx; ++tx)
+                for (int ty = 0; ty <= ay + by; ++ty)
+                    for (int tz = 0; tz <= az + bz; ++tz) row[n++] = ex.e[ax][bx][tx] * ey.e[ay][by][ty] * ez.e[az][bz][tz];
+        }
+}
+void launch_etab(const PairListK &K, const int *lA, const int *lB, double *etab, cudaStream_t st)
+{
+    if (K.n <= 0) return;
+    etab_kernel<<<(K.n + 127) / 128, 128, 0, st>>>(K, lA, lB, etab);
+}
+
 // J_ab = sum_{R2,prims} sum_t (-1)^{|t|} E^{ab}_t J_t  (eq 96-97); one warp per shell pair.
 __global__ void j_backtransform_kernel(PairListU U, ShellInfo sh, const double *__restrict__ Jt, double *__restrict__ Jsr,
                                        int N)
@@ -231,33 +263,56 @@ void launch_agen(const LRParams &p, int g0, int nb, double w0, double *Astack, s
     agen_kernel<<<grid, bs, 0, st>>>(p, g0, nb, w0, Astack, ld);
 }
 
-// rho'[slot] = sum_{mn} P'_mn A'_mn[slot]   (fixed-order block reduction => deterministic)
-__global__ void rho_reduce_kernel(const double *__restrict__ Pp, const double *__restrict__ Astack, size_t ld, int Np, int N,
-                                  double *__restrict__ rho)
+// rho'[slot] = sum_{mn} P'_mn A'_mn[slot]: RHO_CH row chunks per slot, then a fixed-order sum of the
+// chunk partials (deterministic).  HBM-bound: streams the stored batch once.
+constexpr int RHO_CH = 48;
+__global__ void __launch_bounds__(256) rho_reduce_kernel(const double *__restrict__ Pp, const double *__restrict__ Astack,
+                                                         size_t ld, int Np, int N, double *__restrict__ part)
 {
-    const int slot = blockIdx.x;
-    double acc = 0.0;
-    for (int i = threadIdx.x >> 5; i < N; i += (blockDim.x >> 5)) {
+    const int slot = blockIdx.x, ch = blockIdx.y;
+    const int r0 = (int)((long long)N * ch / RHO_CH), r1 = (int)((long long)N * (ch + 1) / RHO_CH);
+    double acc0 = 0.0, acc1 = 0.0;
+    for (int i = r0 + (threadIdx.x >> 5); i < r1; i += 8) {
         const double *a = Astack + (size_t)i * ld + (size_t)slot * Np;
         const double *pr = Pp + (size_t)i * Np;
-        for (int j = threadIdx.x & 31; j < N; j += 32) acc = fma(pr[j], a[j], acc);
+        int j = (threadIdx.x & 31) * 2;
+        for (; j + 1 < N; j += 64) {
+            const double2 av = *reinterpret_cast<const double2 *>(a + j);
+            const double2 pv = *reinterpret_cast<const double2 *>(pr + j);
+            acc0 = fma(pv.x, av.x, acc0);
+            acc1 = fma(pv.y, av.y, acc1);
+        }
+        if (j < N) acc0 = fma(pr[j], a[j], acc0);
     }
-    __shared__ double s[32];
+    double acc = acc0 + acc1;
+    __shared__ double s[8];
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
     if ((threadIdx.x & 31) == 0) s[threadIdx.x >> 5] = acc;
     __syncthreads();
     if (threadIdx.x == 0) {
         double t = 0.0;
-        for (int w = 0; w < (int)(blockDim.x >> 5); ++w) t += s[w];
-        rho[slot] = t;
+        for (int w = 0; w < 8; ++w) t += s[w];
+        part[slot * RHO_CH + ch] = t;
     }
 }
+__global__ void rho_final_kernel(const double *__restrict__ part, int nslot, double *__restrict__ rho)
+{
+    const int slot = blockIdx.x * blockDim.x + threadIdx.x;
+    if (slot >= nslot) return;
+    double t = 0.0;
+    for (int c = 0; c < RHO_CH; ++c) t += part[slot * RHO_CH + c];
+    rho[slot] = t;
+}
+int rho_scratch_doubles(int nslot) { return nslot * (RHO_CH + 1); }
+// rho: nslot results followed by nslot*RHO_CH partials (rho_scratch_doubles)
 void launch_rho_reduce(const double *Pp, const double *Astack, size_t ld, int Np, int N, int nslot, double *rho,
                        cudaStream_t st)
 {
     if (nslot <= 0) return;
-    rho_reduce_kernel<<<nslot, 512, 0, st>>>(Pp, Astack, ld, Np, N, rho);
+    double *part = rho + nslot;
+    rho_reduce_kernel<<<dim3(nslot, RHO_CH), 256, 0, st>>>(Pp, Astack, ld, Np, N, part);
+    rho_final_kernel<<<(nslot + 127) / 128, 128, 0, st>>>(part, nslot, rho);
 }
 
 __global__ void jlr_accum_kernel(const double *__restrict__ Astack, size_t ld, int Np, int N, int nslot,

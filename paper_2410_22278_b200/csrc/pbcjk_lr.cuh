@@ -17,6 +17,8 @@ struct LRParams {
 // P' = f P f (into the padded Np x Np buffer, pads untouched) and ln(max |P'|)
 void launch_scale_density(const double *P, double *Pp, int N, int Np, const double *fcomp,
                           unsigned long long *maxbits, double *lnPmax, cudaStream_t st);
+// E^{AB}_t product table of the ordered pair list (rows at K.eoff), built once per geometry
+void launch_etab(const PairListK &K, const int *lA, const int *lB, double *etab, cudaStream_t st);
 // D~_s of every J ket (eq 95)
 void launch_hermite_density(const PairListU &U, const ShellInfo &sh, const KetListJ &KJ, const double *Pp, int Np,
                             double *Dt, cudaStream_t st);
@@ -27,7 +29,8 @@ void launch_j_backtransform(const PairListU &U, const ShellInfo &sh, const doubl
 // stack  A[row*ld + slot*Np + col], ld = 2*nb_alloc*Np.  g0 < 0: the single G = 0 slot with
 // weight `w0` (overlap S, eq 21), written to slot 0.
 void launch_agen(const LRParams &p, int g0, int nb, double w0, double *Astack, size_t ld, cudaStream_t st);
-// rho'[slot] = sum P' o A'[slot]
+// rho'[slot] = sum P' o A'[slot]; rho must hold rho_scratch_doubles(nslot) doubles (results, then partials)
+int rho_scratch_doubles(int nslot);
 void launch_rho_reduce(const double *Pp, const double *Astack, size_t ld, int Np, int N, int nslot, double *rho,
                        cudaStream_t st);
 // Jacc[m][n] += sign * sum_slot A'[slot][m][n] rho'[slot]

@@ -136,26 +136,15 @@ struct E1D {
     }
 };
 
-// Cartesian powers of component k of a shell with angular momentum l (order xx,xy,xz,yy,yz,zz).
+// Cartesian powers of component k of a shell with angular momentum l <= 2 (order x,y,z / xx,xy,xz,yy,yz,zz:
+// PAPER L721).  Closed forms, so that they fold to constants as soon as k is one (unrolled loops).
 __host__ __device__ constexpr int cart_x(int l, int k)
 {
-    int n = 0;
-    for (int x = l; x >= 0; --x)
-        for (int y = l - x; y >= 0; --y) {
-            if (n == k) return x;
-            ++n;
-        }
-    return 0;
+    return l == 0 ? 0 : (l == 1 ? (k == 0 ? 1 : 0) : (k == 0 ? 2 : (k < 3 ? 1 : 0)));
 }
 __host__ __device__ constexpr int cart_y(int l, int k)
 {
-    int n = 0;
-    for (int x = l; x >= 0; --x)
-        for (int y = l - x; y >= 0; --y) {
-            if (n == k) return y;
-            ++n;
-        }
-    return 0;
+    return l == 0 ? 0 : (l == 1 ? (k == 1 ? 1 : 0) : (k == 3 ? 2 : ((k == 1 || k == 4) ? 1 : 0)));
 }
 __host__ __device__ constexpr int cart_z(int l, int k) { return l - cart_x(l, k) - cart_y(l, k); }
 

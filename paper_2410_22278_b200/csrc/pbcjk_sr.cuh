@@ -218,12 +218,8 @@ __global__ void __launch_bounds__(128) sr_j_kernel(SRParams p, const int *__rest
     }
 }
 
-// ------------------------------------------------------------------------------------------
-// K: class (LA LB | LC LD) with bra = (mu: LA, lambda: LB), ket = (nu: LD, sigma: LC).
-// One CTA owns the output block (mu, nu); warps take the bra primitive pair-images of mu
-// round-robin, lanes the ket primitive pair-images of nu.
-//   K[mu_a, nu_d] += sum P'[lambda_b, sigma_c] (mu_a lambda_b | sigma_c nu_d)      (eq 74)
-// ------------------------------------------------------------------------------------------
+// number of non-zero separable E^{ab}_t over all component pairs of a shell pair (rows of PairListK::etab);
+// the K kernels themselves are in pbcjk_srk.cuh
 template <int LA, int LB>
 __host__ __device__ constexpr int bra_terms()
 {
@@ -233,194 +229,6 @@ __host__ __device__ constexpr int bra_terms()
             n += (cart_x(LA, a) + cart_x(LB, b) + 1) * (cart_y(LA, a) + cart_y(LB, b) + 1) *
                  (cart_z(LA, a) + cart_z(LB, b) + 1);
     return n;
-}
-
-constexpr int KWARPS = 4;
-
-template <int LA, int LB, int LC, int LD>
-__global__ void __launch_bounds__(KWARPS * 32) sr_k_kernel(SRParams p, const int2 *__restrict__ blocks, int nblocks)
-{
-    constexpr int LBRA = LA + LB, LKET = LC + LD, L = LBRA + LKET;
-    constexpr int NA = ncart(LA), NB = ncart(LB), NC = ncart(LC), ND = ncart(LD);
-    constexpr int NTERM = bra_terms<LA, LB>();
-    __shared__ int2 s_queue[KWARPS][QCAP];
-    __shared__ double s_E[KWARPS][NTERM];
-    __shared__ double s_red[KWARPS][NA * ND];
-    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-    const int2 blk = blocks[blockIdx.x];
-    const int mu = blk.x, nu = blk.y;
-    const int b0 = __ldg(p.K.off + mu * 3 + LB), b1 = __ldg(p.K.off + mu * 3 + LB + 1);
-    const int k0 = __ldg(p.K.off + nu * 3 + LC), k1 = __ldg(p.K.off + nu * 3 + LC + 1);
-    if (b1 <= b0 || k1 <= k0) return;
-    const Lattice &lat = p.lat;
-    const double *__restrict__ tab = p.boys;
-    const int N = p.sh.nbf;
-    const double gx = __ldg(p.sh.cx + nu), gy = __ldg(p.sh.cy + nu), gz = __ldg(p.sh.cz + nu);
-    const double kext = __ldg(p.K.ext + nu * 3 + LC), kiqmax = __ldg(p.K.ipmax + nu * 3 + LC);
-    const double lbmax_ket = __ldg(p.K.lb + k0);
-    const double thr0 = *p.lnPmax - p.ln_tau;
-
-    double Kacc[NA * ND];
-#pragma unroll
-    for (int i = 0; i < NA * ND; ++i) Kacc[i] = 0.0;
-    int2 *queue = s_queue[w];
-    double *sE = s_E[w];
-    unsigned ncand = 0, nq = 0;
-    unsigned long long nflush = 0;
-
-    for (int i = b0 + w; i < b1; i += KWARPS) {
-        const double thr = __ldg(p.K.lb + i) + thr0;
-        if (thr + lbmax_ket <= 0.0) break;                  // bras sorted: the rest is weaker
-        const double Pix = __ldg(p.K.Px + i), Piy = __ldg(p.K.Py + i), Piz = __ldg(p.K.Pz + i);
-        const double pi_ = __ldg(p.K.p + i), coefi = __ldg(p.K.coef + i);
-        const double ipi = __ldg(p.K.ip + i);
-        const int aoBi = __ldg(p.K.aoB + i);
-        // bra table: (-1)^{|t|} E^{ab}_t for every component pair, in unrolled order (eq 16)
-        {
-            E1D<LA, LB> ex, ey, ez;
-            const double o2p = 0.5 * ipi;
-            ex.build(__ldg(p.K.PAx + i), __ldg(p.K.PBx + i), o2p);
-            ey.build(__ldg(p.K.PAy + i), __ldg(p.K.PBy + i), o2p);
-            ez.build(__ldg(p.K.PAz + i), __ldg(p.K.PBz + i), o2p);
-            __syncwarp();
-            int n = 0;
-#pragma unroll
-            for (int a = 0; a < NA; ++a)
-#pragma unroll
-                for (int b = 0; b < NB; ++b) {
-                    const int ax = cart_x(LA, a), ay = cart_y(LA, a), az = cart_z(LA, a);
-                    const int bx = cart_x(LB, b), by = cart_y(LB, b), bz = cart_z(LB, b);
-#pragma unroll
-                    for (int tx = 0; tx <= ax + bx; ++tx)
-#pragma unroll
-                        for (int ty = 0; ty <= ay + by; ++ty)
-#pragma unroll
-                            for (int tz = 0; tz <= az + bz; ++tz) {
-                                double v = ex.e[ax][bx][tx] * ey.e[ay][by][ty] * ez.e[az][bz][tz];
-                                if ((tx + ty + tz) & 1) v = -v;
-                                if (lane == (n & 31)) sE[n] = v;
-                                ++n;
-                            }
-                }
-            __syncwarp();
-        }
-        int qn = 0;
-
-        auto eval = [&](int j, int timg) {
-            double Tx, Ty, Tz;
-            unpack_img(timg, lat, Tx, Ty, Tz);
-            const double X = __ldg(p.K.Px + j) + Tx - Pix, Y = __ldg(p.K.Py + j) + Ty - Piy,
-                         Z = __ldg(p.K.Pz + j) + Tz - Piz;
-            const double q = __ldg(p.K.p + j);
-            const double r2 = X * X + Y * Y + Z * Z;
-            const double s = rsqrt(pi_ + q);
-            const double alpha = pi_ * q * s * s;
-            const double th = lat.omega * rsqrt(alpha + lat.omega2);
-            const double alpha_w = alpha * th * th;
-            const double pref = coefi * __ldg(p.K.coef + j) * s;
-            double Rm[L + 1];
-            boys_merged<L>(tab, r2, alpha, alpha_w, th, pref, Rm);
-            double R[nherm(L)];
-            hermite_R<L>(R, Rm, X, Y, Z);
-            // ket tables: first index = nu (LD), second = sigma (LC)
-            E1D<LD, LC> kx, ky, kz;
-            if (LKET > 0) {
-                const double o2q = 0.5 * __ldg(p.K.ip + j);
-                kx.build(__ldg(p.K.PAx + j), __ldg(p.K.PBx + j), o2q);
-                ky.build(__ldg(p.K.PAy + j), __ldg(p.K.PBy + j), o2q);
-                kz.build(__ldg(p.K.PAz + j), __ldg(p.K.PBz + j), o2q);
-            }
-            const double *Prow = p.Pp + (size_t)aoBi * p.ldP + __ldg(p.K.aoB + j);
-#pragma unroll
-            for (int d = 0; d < ND; ++d) {
-#pragma unroll
-                for (int c = 0; c < NC; ++c) {
-                    const int dx = cart_x(LD, d), dy = cart_y(LD, d), dz = cart_z(LD, d);
-                    const int cx = cart_x(LC, c), cy = cart_y(LC, c), cz = cart_z(LC, c);
-                    // X_T = sum_s E^{dc}_s R_{T+s}
-                    double XT[nherm(LBRA)];
-#pragma unroll
-                    for (int t = 0; t < nherm(LBRA); ++t) XT[t] = 0.0;
-#pragma unroll
-                    for (int sx = 0; sx <= dx + cx; ++sx)
-#pragma unroll
-                        for (int sy = 0; sy <= dy + cy; ++sy)
-#pragma unroll
-                            for (int sz = 0; sz <= dz + cz; ++sz) {
-                                double e3 = 1.0;
-                                if (LKET > 0) e3 = kx.e[dx][cx][sx] * ky.e[dy][cy][sy] * kz.e[dz][cz][sz];
-#pragma unroll
-                                for (int tx = 0; tx <= LBRA; ++tx)
-#pragma unroll
-                                    for (int ty = 0; ty <= LBRA - tx; ++ty)
-#pragma unroll
-                                        for (int tz = 0; tz <= LBRA - tx - ty; ++tz)
-                                            XT[hidx(tx, ty, tz)] =
-                                                fma(e3, R[hidx(tx + sx, ty + sy, tz + sz)], XT[hidx(tx, ty, tz)]);
-                            }
-                    // I_ab = sum_T (-1)^{|T|} E^{ab}_T X_T ;  K_ad += P'_bc I_ab
-                    int n = 0;
-#pragma unroll
-                    for (int a = 0; a < NA; ++a) {
-                        double kad = Kacc[a * ND + d];
-#pragma unroll
-                        for (int b = 0; b < NB; ++b) {
-                            const int ax = cart_x(LA, a), ay = cart_y(LA, a), az = cart_z(LA, a);
-                            const int bx = cart_x(LB, b), by = cart_y(LB, b), bz = cart_z(LB, b);
-                            double I = 0.0;
-#pragma unroll
-                            for (int tx = 0; tx <= ax + bx; ++tx)
-#pragma unroll
-                                for (int ty = 0; ty <= ay + by; ++ty)
-#pragma unroll
-                                    for (int tz = 0; tz <= az + bz; ++tz) {
-                                        I = fma(sE[n], XT[hidx(tx, ty, tz)], I);
-                                        ++n;
-                                    }
-                            kad = fma(__ldg(Prow + (size_t)b * p.ldP + c), I, kad);
-                        }
-                        Kacc[a * ND + d] = kad;
-                    }
-                }
-            }
-        };
-
-        scan_group(lat, Pix, Piy, Piz, ipi, thr, gx, gy, gz, kext, kiqmax, k0, k1, p.K.Px, p.K.Py, p.K.Pz,
-                   p.K.ip, p.K.lb, p.rcut2, queue, qn, lane, ncand, nq, eval);
-        if (qn > 0) {
-            if (lane < qn) {
-                const int2 e = queue[lane];
-                eval(e.x, e.y);
-            }
-            nflush += qn;
-        }
-        __syncwarp();
-    }
-    // warp shuffle reduction, then shared-memory reduction across the CTA's warps
-#pragma unroll
-    for (int i = 0; i < NA * ND; ++i) {
-        double v = Kacc[i];
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-        if (lane == 0) s_red[w][i] = v;
-    }
-    __syncthreads();
-    if (threadIdx.x < NA * ND) {
-        double v = 0.0;
-#pragma unroll
-        for (int ww = 0; ww < KWARPS; ++ww) v += s_red[ww][threadIdx.x];
-        const int a = threadIdx.x / ND, d = threadIdx.x % ND;
-        double *dst = p.Ksr + (size_t)(__ldg(p.sh.ao + mu) + a) * N + __ldg(p.sh.ao + nu) + d;
-        *dst += v;                                          // this CTA is the only owner of the block
-    }
-    unsigned long long c = ncand;
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) c += __shfl_xor_sync(0xffffffffu, c, o);
-    if (lane == 0) {
-        constexpr int cls = ((LA * 3 + LB) * 3 + LC) * 3 + LD;
-        atomicAdd(p.counters + CNT_CAND_K + cls, c);
-        atomicAdd(p.counters + CNT_Q_K + cls, (unsigned long long)nq * 32ull + nflush);
-    }
 }
 
 // launchers (defined in the instantiation units)
