@@ -77,44 +77,63 @@ __device__ __forceinline__ void scan_group(const Lattice &lat, double Pix, doubl
     const int lo1 = (int)ceil(f1 - rho * lat.bnorm[1]), hi1 = (int)floor(f1 + rho * lat.bnorm[1]);
     const int lo2 = (int)ceil(f2 - rho * lat.bnorm[2]), hi2 = (int)floor(f2 + rho * lat.bnorm[2]);
     const unsigned ltmask = (1u << lane) - 1u;
-    for (int n0 = lo0; n0 <= hi0; ++n0)
-        for (int n1 = lo1; n1 <= hi1; ++n1)
-            for (int n2 = lo2; n2 <= hi2; ++n2) {
-                const double Tx = n0 * lat.a[0] + n1 * lat.a[3] + n2 * lat.a[6];
-                const double Ty = n0 * lat.a[1] + n1 * lat.a[4] + n2 * lat.a[7];
-                const double Tz = n0 * lat.a[2] + n1 * lat.a[5] + n2 * lat.a[8];
-                const double ex = Tx - cx, ey = Ty - cy, ez = Tz - cz;
-                const double dist2 = ex * ex + ey * ey + ez * ez;
-                if (dist2 > rho * rho) continue;
-                double dlb = sqrt(dist2) - ext;                 // lower bound of |Q + T - P|
-                dlb = dlb > 0.0 ? dlb : 0.0;
-                const double need = dlb * dlb / isum_max - thr; // ket survives only if lb_ket > need
-                const int timg = pack_img(n0, n1, n2);
-                const double ox = Tx - Pix, oy = Ty - Piy, oz = Tz - Piz;
-                for (int j0 = k0; j0 < k1; j0 += 32) {
-                    if (__ldg(klb + j0) <= need) break;         // sorted: nothing further survives
-                    const int j = j0 + lane;
-                    bool pass = false;
-                    if (j < k1) {
-                        const double dx = __ldg(kQx + j) + ox, dy = __ldg(kQy + j) + oy, dz = __ldg(kQz + j) + oz;
-                        const double r2 = dx * dx + dy * dy + dz * dz;
-                        const double isum = ipi + __ldg(kiq + j) + lat.iomega2;
-                        pass = (thr + __ldg(klb + j)) * isum > r2 && r2 <= rcut2;
-                        ++ncand;
-                    }
-                    const unsigned m = __ballot_sync(0xffffffffu, pass);
-                    if (pass) queue[qn + __popc(m & ltmask)] = make_int2(j, timg);
-                    qn += __popc(m);
+    const int d1 = hi1 - lo1 + 1, d2 = hi2 - lo2 + 1, d12 = d1 * d2;
+    const int nimg = (hi0 >= lo0 && d1 > 0 && d2 > 0) ? (hi0 - lo0 + 1) * d12 : 0;
+    const double inv_isum_max = 1.0 / isum_max, rho2 = rho * rho;
+    for (int base = 0; base < nimg; base += 32) {
+        // 32 images of the box at a time, one per lane: sphere filter and the bound a ket needs there
+        const int im = base + lane;
+        bool ok = false;
+        double need_l = 0.0;
+        int timg_l = 0;
+        if (im < nimg) {
+            const int n0 = lo0 + im / d12, r = im % d12;
+            const int n1 = lo1 + r / d2, n2 = lo2 + r % d2;
+            const double Tx = n0 * lat.a[0] + n1 * lat.a[3] + n2 * lat.a[6];
+            const double Ty = n0 * lat.a[1] + n1 * lat.a[4] + n2 * lat.a[7];
+            const double Tz = n0 * lat.a[2] + n1 * lat.a[5] + n2 * lat.a[8];
+            const double ex = Tx - cx, ey = Ty - cy, ez = Tz - cz;
+            const double dist2 = ex * ex + ey * ey + ez * ez;
+            ok = dist2 <= rho2;
+            double dlb = sqrt(dist2) - ext;                     // lower bound of |Q + T - P|
+            dlb = dlb > 0.0 ? dlb : 0.0;
+            need_l = dlb * dlb * inv_isum_max - thr;            // ket survives only if lb_ket > need
+            timg_l = pack_img(n0, n1, n2);
+        }
+        unsigned imask = __ballot_sync(0xffffffffu, ok);
+        while (imask) {
+            const int src = __ffs(imask) - 1;
+            imask &= imask - 1;
+            const double need = __shfl_sync(0xffffffffu, need_l, src);
+            const int timg = __shfl_sync(0xffffffffu, timg_l, src);
+            double Tx, Ty, Tz;
+            unpack_img(timg, lat, Tx, Ty, Tz);
+            const double ox = Tx - Pix, oy = Ty - Piy, oz = Tz - Piz;
+            for (int j0 = k0; j0 < k1; j0 += 32) {
+                if (__ldg(klb + j0) <= need) break;             // sorted: nothing further survives
+                const int j = j0 + lane;
+                bool pass = false;
+                if (j < k1) {
+                    const double dx = __ldg(kQx + j) + ox, dy = __ldg(kQy + j) + oy, dz = __ldg(kQz + j) + oz;
+                    const double r2 = dx * dx + dy * dy + dz * dz;
+                    const double isum = ipi + __ldg(kiq + j) + lat.iomega2;
+                    pass = (thr + __ldg(klb + j)) * isum > r2 && r2 <= rcut2;
+                    ++ncand;
+                }
+                const unsigned m = __ballot_sync(0xffffffffu, pass);
+                if (pass) queue[qn + __popc(m & ltmask)] = make_int2(j, timg);
+                qn += __popc(m);
+                __syncwarp();
+                if (qn >= 32) {
+                    qn -= 32;
+                    const int2 e = queue[qn + lane];
                     __syncwarp();
-                    if (qn >= 32) {
-                        qn -= 32;
-                        const int2 e = queue[qn + lane];
-                        __syncwarp();
-                        eval(e.x, e.y);
-                        ++nq;
-                    }
+                    eval(e.x, e.y);
+                    ++nq;
                 }
             }
+        }
+    }
 }
 
 // ------------------------------------------------------------------------------------------

@@ -93,31 +93,52 @@ sr_k_kernel(SRParams p, const int2 *__restrict__ blocks, int nblocks)
         const int lo2 = (int)ceil(f2 - rho * lat.bnorm[2]), hi2 = (int)floor(f2 + rho * lat.bnorm[2]);
         const int d1 = hi1 - lo1 + 1, d2 = hi2 - lo2 + 1;
         const int nimg = (hi0 >= lo0 && d1 > 0 && d2 > 0) ? (hi0 - lo0 + 1) * d1 * d2 : 0;
-        int img = 0, j0 = k0, qn = 0, timg = 0;
+        const double inv_isum_max = 1.0 / isum_max, rho2 = rho * rho;
+        const int d12 = d1 * d2;
+        int base = 0, j0 = k0, qn = 0, timg = 0, timg_l = 0;
+        unsigned imask = 0;                                 // images of the current batch still to visit
         bool have = false;
-        double need = 0.0, ox = 0.0, oy = 0.0, oz = 0.0;
+        double need = 0.0, need_l = 0.0, ox = 0.0, oy = 0.0, oz = 0.0;
 
         for (;;) {
             // ---- phase 1: screen (ket, image) candidates until 32 survivors are queued ----
-            while (qn < 32 && img < nimg) {
+            while (qn < 32) {
                 if (!have) {
-                    const int n0 = lo0 + img / (d1 * d2), r = img % (d1 * d2);
-                    const int n1 = lo1 + r / d2, n2 = lo2 + r % d2;
-                    const double Tx = n0 * lat.a[0] + n1 * lat.a[3] + n2 * lat.a[6];
-                    const double Ty = n0 * lat.a[1] + n1 * lat.a[4] + n2 * lat.a[7];
-                    const double Tz = n0 * lat.a[2] + n1 * lat.a[5] + n2 * lat.a[8];
-                    const double ex = Tx - cx, ey = Ty - cy, ez = Tz - cz;
-                    const double dist2 = ex * ex + ey * ey + ez * ez;
-                    if (dist2 > rho * rho) { ++img; continue; }
-                    double dlb = sqrt(dist2) - kext;            // lower bound of |Q + T - P|
-                    dlb = dlb > 0.0 ? dlb : 0.0;
-                    need = dlb * dlb / isum_max - thr;          // a ket survives only if lb_ket > need
-                    timg = pack_img(n0, n1, n2);
+                    if (imask == 0) {
+                        if (base >= nimg) break;
+                        // 32 images of the box at a time, one per lane: sphere filter and the bound each
+                        // image needs from a ket (eq 67 with the closest approach of the ket group)
+                        const int im = base + lane;
+                        base += 32;
+                        bool ok = false;
+                        if (im < nimg) {
+                            const int n0 = lo0 + im / d12, r = im % d12;
+                            const int n1 = lo1 + r / d2, n2 = lo2 + r % d2;
+                            const double Tx = n0 * lat.a[0] + n1 * lat.a[3] + n2 * lat.a[6];
+                            const double Ty = n0 * lat.a[1] + n1 * lat.a[4] + n2 * lat.a[7];
+                            const double Tz = n0 * lat.a[2] + n1 * lat.a[5] + n2 * lat.a[8];
+                            const double ex = Tx - cx, ey = Ty - cy, ez = Tz - cz;
+                            const double dist2 = ex * ex + ey * ey + ez * ez;
+                            ok = dist2 <= rho2;
+                            double dlb = sqrt(dist2) - kext;    // lower bound of |Q + T - P|
+                            dlb = dlb > 0.0 ? dlb : 0.0;
+                            need_l = dlb * dlb * inv_isum_max - thr;   // a ket survives only if lb_ket > need
+                            timg_l = pack_img(n0, n1, n2);
+                        }
+                        imask = __ballot_sync(0xffffffffu, ok);
+                        continue;
+                    }
+                    const int src = __ffs(imask) - 1;
+                    imask &= imask - 1;
+                    need = __shfl_sync(0xffffffffu, need_l, src);
+                    timg = __shfl_sync(0xffffffffu, timg_l, src);
+                    double Tx, Ty, Tz;
+                    unpack_img(timg, lat, Tx, Ty, Tz);
                     ox = Tx - Pix; oy = Ty - Piy; oz = Tz - Piz;
                     j0 = k0;
                     have = true;
                 }
-                if (j0 >= k1 || __ldg(klb + j0) <= need) { ++img; have = false; continue; }   // sorted by lb
+                if (j0 >= k1 || __ldg(klb + j0) <= need) { have = false; continue; }   // sorted by lb
                 const int j = j0 + lane;
                 bool pass = false;
                 if (j < k1) {
