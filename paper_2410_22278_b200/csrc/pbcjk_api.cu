@@ -82,7 +82,8 @@ struct pbc_jk {
     double *LT = nullptr, *chol_d = nullptr, *chol_s = nullptr;      // factor P' = L L^T of the K^LR contraction
     int *chol_dyn = nullptr;
     unsigned long long *maxbits = nullptr, *counters = nullptr;
-    int nb = 1, nsplit = 1;
+    int nb = 1, nsplit = 1, Smax = 16;
+    int cur_S = 0;                       // slot count the A' stack is currently laid out (and zero-filled) for
     bool has_l[LMAX + 1] = {};
     size_t ld = 0;
     double c0 = 0.0;             // pi/(Omega w^2)
@@ -470,6 +471,14 @@ int setup(pbc_jk *h, const pbc_cell *cell, const pbc_atoms *atoms, const pbc_she
         CK(pool.upload(&U.PBx, soa(up, 6, 0))); CK(pool.upload(&U.PBy, soa(up, 6, 1))); CK(pool.upload(&U.PBz, soa(up, 6, 2)));
         CK(pool.upload(&U.sp, u_sp)); CK(pool.upload(&U.sp_off, sp_off));
         CK(pool.upload(&U.sp_shA, sp_shA)); CK(pool.upload(&U.sp_shB, sp_shB));
+        // shell pairs by class (l_A, l_B): one rho_mn(G) kernel instantiation per class
+        for (int c = 0; c < 9; ++c) {
+            std::vector<int> lst;
+            for (size_t q = 0; q < sp_shA.size(); ++q)
+                if (sh_l[sp_shA[q]] * 3 + sh_l[sp_shB[q]] == c) lst.push_back((int)q);
+            CK(pool.upload(&h->lr.sp_cls[c], lst));
+            h->lr.n_sp_cls[c] = (int)lst.size();
+        }
         // J bra lists per Hermite order, heaviest first
         for (int LB = 0; LB <= 4; ++LB) {
             std::vector<int> b;
@@ -560,9 +569,10 @@ int setup(pbc_jk *h, const pbc_cell *cell, const pbc_atoms *atoms, const pbc_she
         const size_t Np = h->Np, N = nbf;
         // G batch: A' and Y stacks of Np x 2nb x Np doubles each, at most 12 GB per stack (180 GB HBM3e per GPU)
         int nb = cut.lr_g_batch > 0 ? cut.lr_g_batch : (int)std::min<double>(64.0, std::floor(12.0e9 / (double)(Np * Np * 16)));
-        nb = std::max(1, std::min(nb, std::max(h->nG, 1)));
+        nb = std::max(1, std::min(std::min(nb, 64), std::max(h->nG, 1)));      // the slot kernels hold at most 128 slots
         h->nb = nb;
-        h->ld = (size_t)2 * nb * Np;
+        h->Smax = ((2 * nb + 15) / 16) * 16;             // slots of a full batch (multiple of 16)
+        h->ld = (size_t)h->Smax * Np;
         h->nsplit = Np <= 2048 ? 4 : 1;
         CK(pool.alloc(&h->Pp, Np * Np)); CK(cudaMemset(h->Pp, 0, Np * Np * 8));
         CK(pool.alloc(&h->lnPmax, 1)); CK(pool.alloc(&h->maxbits, 1));
@@ -573,7 +583,7 @@ int setup(pbc_jk *h, const pbc_cell *cell, const pbc_atoms *atoms, const pbc_she
         CK(pool.alloc(&h->Klr, (size_t)h->nsplit * Np * Np));
         CK(pool.alloc(&h->Astack, Np * h->ld)); CK(cudaMemset(h->Astack, 0, Np * h->ld * 8));
         CK(pool.alloc(&h->Zstack, Np * h->ld));
-        CK(pool.alloc(&h->rho, (size_t)rho_scratch_doubles(2 * nb)));
+        CK(pool.alloc(&h->rho, (size_t)rho_scratch_doubles(h->Smax)));
         CK(pool.alloc(&h->LT, Np * Np)); CK(pool.alloc(&h->chol_d, 2 * Np)); CK(pool.alloc(&h->chol_s, 2));
         CK(pool.alloc(&h->chol_dyn, 4));
         CK(pool.alloc(&h->hostP, N * N)); CK(pool.alloc(&h->hostJ, N * N)); CK(pool.alloc(&h->hostK, N * N));
@@ -583,9 +593,10 @@ int setup(pbc_jk *h, const pbc_cell *cell, const pbc_atoms *atoms, const pbc_she
     }
     // ---- A3: overlap S = rho_mn(G = 0) (eq 21) ----
     {
-        launch_agen(h->lr, -1, 1, 1.0, h->Astack, h->ld, 0);
+        h->cur_S = 16;                   // the whole stack was zero-filled at allocation
+        launch_agen(h->lr, -1, 1, 16, 1.0, h->Astack, 0);
         double *dS = h->hostJ;
-        launch_extract_overlap(h->Astack, h->ld, nbf, h->fcomp, dS, 0);
+        launch_extract_overlap(h->Astack, h->Np, 16, nbf, h->fcomp, dS, 0);
         h->S_host.resize((size_t)nbf * nbf);
         CK(cudaMemcpy(h->S_host.data(), dS, (size_t)nbf * nbf * 8, cudaMemcpyDeviceToHost));
         CK(cudaGetLastError());
@@ -725,39 +736,52 @@ int pbc_jk_build(pbc_jk *h, const double *P, double *J, double *K, void *cuda_st
         launch_factor_density(h->Pp, N, Np, h->LT, h->chol_d, h->chol_dyn, h->chol_s, h->Zstack, st);
         nl += factor_density_launches(N);
     }
-    auto klr_batch = [&](int nslot, double alpha, int nsplit) {
-        GemmArgs g1;                                     // Y = L^T [A'_1 A'_2 ...]  (rows >= rank skipped)
-        g1.M = Np; g1.Nc = nslot * Np; g1.Kb = Np; g1.nbatch = 1; g1.A = h->LT; g1.lda = Np; g1.B = h->Astack; g1.ldb = h->ld;
-        g1.C = h->Zstack; g1.ldc = h->ld; g1.dyn = h->chol_dyn; g1.use_dyn = 1;
+    // one batch of S slots (layout A'[row*Np*S + col*S + slot]):  Y = L^T A'  (rows >= rank skipped), then
+    // K += alpha sum_r sum_slot Y[r][mu][slot] Y[r][nu][slot] on the lower tiles (batches = rows r of the factor)
+    auto klr_batch = [&](int S, double alpha, int nsplit) {
+        const size_t ldS = (size_t)Np * S;
+        GemmArgs g1;
+        g1.M = Np; g1.Nc = Np * S; g1.Kb = Np; g1.nbatch = 1; g1.A = h->LT; g1.lda = Np; g1.B = h->Astack; g1.ldb = ldS;
+        g1.C = h->Zstack; g1.ldc = ldS; g1.dyn = h->chol_dyn; g1.use_dyn = 1;
         launch_dgemm(g1, st);
-        GemmArgs g2;                                     // K += alpha sum_slot Y_slot^T Y_slot  (lower tiles)
-        g2.M = Np; g2.Nc = Np; g2.Kb = Np; g2.nbatch = nslot; g2.alpha = alpha; g2.transA = true;
-        g2.A = h->Zstack; g2.lda = h->ld; g2.strideA = Np; g2.B = h->Zstack; g2.ldb = h->ld; g2.strideB = Np;
+        GemmArgs g2;
+        g2.M = Np; g2.Nc = Np; g2.Kb = S; g2.nbatch = Np; g2.alpha = alpha; g2.transB = true;
+        g2.A = h->Zstack; g2.lda = S; g2.strideA = ldS; g2.B = h->Zstack; g2.ldb = S; g2.strideB = ldS;
         g2.B_alt = h->Astack; g2.beta = 1.0; g2.C = h->Klr; g2.ldc = Np; g2.strideC = strideK; g2.nsplit = nsplit;
-        g2.dyn = h->chol_dyn; g2.use_dyn = 2 | 4; g2.lower_only = 1;
+        g2.dyn = h->chol_dyn; g2.use_dyn = 4 | 8; g2.lower_only = 1;
         launch_dgemm(g2, st);
+    };
+    const int n_agen = agen_launches(h->lr);
+    // Elements of shell pairs with no primitive pair-image are never written by agen_kernel and must read as 0:
+    // the stack is zero-filled whenever its layout (the slot count S) changes.
+    auto set_layout = [&](int S) -> cudaError_t {
+        if (h->cur_S == S) return cudaSuccess;
+        h->cur_S = S;
+        return cudaMemsetAsync(h->Astack, 0, (size_t)Np * Np * S * sizeof(double), st);
     };
     if (doLR) {
         for (int g0 = 0; g0 < h->nG; g0 += h->nb) {
-            const int nb = std::min(h->nb, h->nG - g0), nslot = 2 * nb;
-            launch_agen(h->lr, g0, nb, 0.0, h->Astack, h->ld, st);
-            nl += 1 + (J ? 3 : 0) + (K ? 2 : 0);
+            const int nb = std::min(h->nb, h->nG - g0), S = ((2 * nb + 15) / 16) * 16;
+            CK(set_layout(S));
+            launch_agen(h->lr, g0, nb, S, 0.0, h->Astack, st);
+            nl += n_agen + (J ? 3 : 0) + (K ? 2 : 0);
             if (J) {
-                launch_rho_reduce(h->Pp, h->Astack, h->ld, Np, N, nslot, h->rho, st);
-                launch_jlr_accum(h->Astack, h->ld, Np, N, nslot, h->rho, 1.0, h->Jlr, st);
+                launch_rho_reduce(h->Pp, h->Astack, Np, N, S, h->rho, st);
+                launch_jlr_accum(h->Astack, Np, N, S, h->rho, 1.0, h->Jlr, st);
             }
-            if (K) klr_batch(nslot, 1.0, std::min(h->nsplit, nslot));
+            if (K) klr_batch(S, 1.0, h->nsplit);
         }
     }
     // ---- A9: the G = 0 slot, weight -pi/(Omega w^2), A = S ----
     if (doSELF) {
-        launch_agen(h->lr, -1, 1, std::sqrt(h->c0), h->Astack, h->ld, st);
-        nl += 1 + (J ? 3 : 0) + (K ? 2 : 0);
+        CK(set_layout(16));
+        launch_agen(h->lr, -1, 1, 16, std::sqrt(h->c0), h->Astack, st);
+        nl += n_agen + (J ? 3 : 0) + (K ? 2 : 0);
         if (J) {
-            launch_rho_reduce(h->Pp, h->Astack, h->ld, Np, N, 1, h->rho, st);
-            launch_jlr_accum(h->Astack, h->ld, Np, N, 1, h->rho, -1.0, h->Jlr, st);
+            launch_rho_reduce(h->Pp, h->Astack, Np, N, 16, h->rho, st);
+            launch_jlr_accum(h->Astack, Np, N, 16, h->rho, -1.0, h->Jlr, st);
         }
-        if (K) klr_batch(1, -1.0, 1);
+        if (K) klr_batch(16, -1.0, h->nsplit);
     }
     CK(cudaEventRecord(h->ev[4], st));
     // ---- A10 ----

@@ -178,159 +178,186 @@ void launch_j_backtransform(const PairListU &U, const ShellInfo &sh, const doubl
 }
 
 // ---------------------------------------------------------------- rho_mn(G) generation (A7)
-// thread = (shell pair, G of the batch).  Writes the block and its mirror (rho_mn = rho_nm).
-__global__ void agen_kernel(LRParams p, int g0, int nb, double w0, double *__restrict__ Astack, size_t ld)
+// Stack layout (slot fastest): A'[row*ld + col*S + slot], ld = Np*S, S = slots of the batch rounded up to 16
+// (slot 2g = Re, 2g+1 = Im of G number g of the batch, weight sqrt(w) folded in; slots past the batch are 0).
+// One block per shell pair of class (LA, LB), threads over the G of the batch: each thread writes its (Re, Im)
+// pair as one 16-byte store, so a warp writes 512 contiguous bytes per matrix element.
+template <int LA, int LB>
+__global__ void __launch_bounds__(64) agen_kernel(LRParams p, const int *__restrict__ sp_list, int g0, int nb, int S, double w0,
+                                                  double *__restrict__ Astack, size_t ld)
 {
-    const int sp = blockIdx.x;
+    constexpr int NA = ncart(LA), NB = ncart(LB);
+    const int sp = sp_list[blockIdx.x];
     const int gl = blockIdx.y * blockDim.x + threadIdx.x;
-    if (gl >= nb) return;
+    if (2 * gl >= S) return;
     const bool overlap = g0 < 0;
-    double Gx = 0, Gy = 0, Gz = 0, sw = w0;
-    if (!overlap) {
+    const bool live = gl < nb;
+    double Gx = 0, Gy = 0, Gz = 0, sw = live ? w0 : 0.0;
+    if (!overlap && live) {
         Gx = p.Gx[g0 + gl]; Gy = p.Gy[g0 + gl]; Gz = p.Gz[g0 + gl]; sw = p.Gw[g0 + gl];
     }
     const double G2 = Gx * Gx + Gy * Gy + Gz * Gz;
     const PairListU &U = p.U;
     const int A = U.sp_shA[sp], B = U.sp_shB[sp];
-    const int la = p.sh.l[A], lb = p.sh.l[B];
-    const int na = ncart(la), nbc = ncart(lb);
-    double accr[36], acci[36];
-    for (int i = 0; i < 36; ++i) { accr[i] = 0.0; acci[i] = 0.0; }
-    for (int u = U.sp_off[sp]; u < U.sp_off[sp + 1]; ++u) {
-        const double pp = U.p[u], ip = U.ip[u];
-        // coef holds sqrt2 pi^{5/4}/p; the transform needs (pi/p)^{3/2}
-        const double cft = U.coef[u] * 0.94139626377671481 * rsqrt(pp) * exp(-0.25 * G2 * ip) * sw;
-        double sn, cs;
-        sincos(-(Gx * U.Px[u] + Gy * U.Py[u] + Gz * U.Pz[u]), &sn, &cs);
-        const double phr = cft * cs, phi = cft * sn;
-        E1Drt ex, ey, ez;
-        const double o2p = 0.5 * ip;
-        ex.build(la, lb, U.PAx[u], U.PBx[u], o2p);
-        ey.build(la, lb, U.PAy[u], U.PBy[u], o2p);
-        ez.build(la, lb, U.PAz[u], U.PBz[u], o2p);
-        // per direction: S[i][j] = sum_t E^{ij}_t (-iG)^t
-        double sr[3][LMAX + 1][LMAX + 1], si[3][LMAX + 1][LMAX + 1];
-        for (int d = 0; d < 3; ++d) {
-            const E1Drt &e = d == 0 ? ex : (d == 1 ? ey : ez);
-            const double g = d == 0 ? Gx : (d == 1 ? Gy : Gz);
-            for (int i = 0; i <= la; ++i)
-                for (int j = 0; j <= lb; ++j) {
-                    double r = 0.0, im = 0.0, gp = 1.0;
-                    for (int t = 0; t <= i + j; ++t) {
-                        const double v = e.e[i][j][t] * gp;        // (-i)^t: 1, -i, -1, i
-                        switch (t & 3) {
-                        case 0: r += v; break;
-                        case 1: im -= v; break;
-                        case 2: r -= v; break;
-                        default: im += v; break;
-                        }
-                        gp *= g;
+    double accr[NA * NB], acci[NA * NB];
+#pragma unroll
+    for (int i = 0; i < NA * NB; ++i) { accr[i] = 0.0; acci[i] = 0.0; }
+    if (live) {
+        const double g[3] = {Gx, Gy, Gz};
+        for (int u = U.sp_off[sp]; u < U.sp_off[sp + 1]; ++u) {
+            const double pp = U.p[u], ip = U.ip[u];
+            // coef holds sqrt2 pi^{5/4}/p; the transform needs (pi/p)^{3/2}
+            const double cft = U.coef[u] * 0.94139626377671481 * rsqrt(pp) * exp(-0.25 * G2 * ip) * sw;
+            double sn, cs;
+            sincos(-(Gx * U.Px[u] + Gy * U.Py[u] + Gz * U.Pz[u]), &sn, &cs);
+            const double phr = cft * cs, phi = cft * sn;
+            const double o2p = 0.5 * ip;
+            const double PA[3] = {U.PAx[u], U.PAy[u], U.PAz[u]}, PB[3] = {U.PBx[u], U.PBy[u], U.PBz[u]};
+            // per direction: s[i][j] = sum_t E^{ij}_t (-iG)^t
+            double sr[3][LA + 1][LB + 1], si[3][LA + 1][LB + 1];
+#pragma unroll
+            for (int d = 0; d < 3; ++d) {
+                E1D<LA, LB> e;
+                e.build(PA[d], PB[d], o2p);
+                const double g1 = g[d], g2 = g1 * g1;
+#pragma unroll
+                for (int i = 0; i <= LA; ++i)
+#pragma unroll
+                    for (int j = 0; j <= LB; ++j) {
+                        double r = e.e[i][j][0], im = 0.0;            // (-i)^t: 1, -i, -1, i
+                        if (i + j >= 1) im = -e.e[i][j][1] * g1;
+                        if (i + j >= 2) r = fma(-e.e[i][j][2], g2, r);
+                        if (i + j >= 3) im = fma(e.e[i][j][3], g2 * g1, im);
+                        if (i + j >= 4) r = fma(e.e[i][j][4], g2 * g2, r);
+                        sr[d][i][j] = r; si[d][i][j] = im;
                     }
-                    sr[d][i][j] = r; si[d][i][j] = im;
+            }
+#pragma unroll
+            for (int a = 0; a < NA; ++a)
+#pragma unroll
+                for (int b = 0; b < NB; ++b) {
+                    const int ax = cart_x(LA, a), ay = cart_y(LA, a), az = cart_z(LA, a);
+                    const int bx = cart_x(LB, b), by = cart_y(LB, b), bz = cart_z(LB, b);
+                    double r = sr[0][ax][bx], im = si[0][ax][bx];
+                    const double r2 = r * sr[1][ay][by] - im * si[1][ay][by], i2 = r * si[1][ay][by] + im * sr[1][ay][by];
+                    r = r2 * sr[2][az][bz] - i2 * si[2][az][bz];
+                    im = r2 * si[2][az][bz] + i2 * sr[2][az][bz];
+                    accr[a * NB + b] += r * phr - im * phi;
+                    acci[a * NB + b] += r * phi + im * phr;
                 }
         }
-        for (int a = 0; a < na; ++a)
-            for (int b = 0; b < nbc; ++b) {
-                int ax, ay, az, bx, by, bz;
-                cart_powers(la, a, ax, ay, az);
-                cart_powers(lb, b, bx, by, bz);
-                double r = sr[0][ax][bx], im = si[0][ax][bx];
-                double r2 = r * sr[1][ay][by] - im * si[1][ay][by], i2 = r * si[1][ay][by] + im * sr[1][ay][by];
-                r = r2 * sr[2][az][bz] - i2 * si[2][az][bz];
-                im = r2 * si[2][az][bz] + i2 * sr[2][az][bz];
-                accr[a * nbc + b] += r * phr - im * phi;
-                acci[a * nbc + b] += r * phi + im * phr;
-            }
     }
     const int oa = p.sh.ao[A], ob = p.sh.ao[B];
-    const size_t slot_r = overlap ? 0 : (size_t)(2 * gl), slot_i = slot_r + 1;
-    for (int a = 0; a < na; ++a)
-        for (int b = 0; b < nbc; ++b) {
-            const double vr = accr[a * nbc + b], vi = acci[a * nbc + b];
-            Astack[(size_t)(oa + a) * ld + slot_r * p.Np + ob + b] = vr;
-            Astack[(size_t)(ob + b) * ld + slot_r * p.Np + oa + a] = vr;
-            if (!overlap) {
-                Astack[(size_t)(oa + a) * ld + slot_i * p.Np + ob + b] = vi;
-                Astack[(size_t)(ob + b) * ld + slot_i * p.Np + oa + a] = vi;
-            }
+#pragma unroll
+    for (int a = 0; a < NA; ++a)
+#pragma unroll
+        for (int b = 0; b < NB; ++b) {
+            const double2 v = make_double2(accr[a * NB + b], overlap ? 0.0 : acci[a * NB + b]);
+            *reinterpret_cast<double2 *>(Astack + (size_t)(oa + a) * ld + (size_t)(ob + b) * S + 2 * gl) = v;
+            *reinterpret_cast<double2 *>(Astack + (size_t)(ob + b) * ld + (size_t)(oa + a) * S + 2 * gl) = v;
         }
 }
-void launch_agen(const LRParams &p, int g0, int nb, double w0, double *Astack, size_t ld, cudaStream_t st)
+template <int LA, int LB>
+static void launch_agen_class(const LRParams &p, int g0, int nb, int S, double w0, double *Astack, size_t ld, cudaStream_t st)
+{
+    const int n = p.n_sp_cls[LA * 3 + LB];
+    if (n <= 0) return;
+    dim3 grid(n, (S / 2 + 63) / 64);
+    agen_kernel<LA, LB><<<grid, 64, 0, st>>>(p, p.sp_cls[LA * 3 + LB], g0, nb, S, w0, Astack, ld);
+}
+int agen_launches(const LRParams &p)
+{
+    int n = 0;
+    for (int c = 0; c < 9; ++c) n += p.n_sp_cls[c] > 0;
+    return n;
+}
+void launch_agen(const LRParams &p, int g0, int nb, int S, double w0, double *Astack, cudaStream_t st)
 {
     if (p.U.nsp <= 0 || nb <= 0) return;
-    const int bs = nb >= 64 ? 64 : 32;
-    dim3 grid(p.U.nsp, (nb + bs - 1) / bs);
-    agen_kernel<<<grid, bs, 0, st>>>(p, g0, nb, w0, Astack, ld);
+    const size_t ld = (size_t)p.Np * S;
+    launch_agen_class<0, 0>(p, g0, nb, S, w0, Astack, ld, st); launch_agen_class<0, 1>(p, g0, nb, S, w0, Astack, ld, st);
+    launch_agen_class<0, 2>(p, g0, nb, S, w0, Astack, ld, st); launch_agen_class<1, 0>(p, g0, nb, S, w0, Astack, ld, st);
+    launch_agen_class<1, 1>(p, g0, nb, S, w0, Astack, ld, st); launch_agen_class<1, 2>(p, g0, nb, S, w0, Astack, ld, st);
+    launch_agen_class<2, 0>(p, g0, nb, S, w0, Astack, ld, st); launch_agen_class<2, 1>(p, g0, nb, S, w0, Astack, ld, st);
+    launch_agen_class<2, 2>(p, g0, nb, S, w0, Astack, ld, st);
 }
 
-// rho'[slot] = sum_{mn} P'_mn A'_mn[slot]: RHO_CH row chunks per slot, then a fixed-order sum of the
-// chunk partials (deterministic).  HBM-bound: streams the stored batch once.
-constexpr int RHO_CH = 48;
+// rho'[slot] = sum_{mn} P'_mn A'_mn[slot]: RHO_CH row chunks, threads over the (contiguous) slots, then a
+// fixed-order sum of the chunk partials (deterministic).  HBM-bound: streams the stored batch once.
+constexpr int RHO_CH = 296;
 __global__ void __launch_bounds__(256) rho_reduce_kernel(const double *__restrict__ Pp, const double *__restrict__ Astack,
-                                                         size_t ld, int Np, int N, double *__restrict__ part)
+                                                         size_t ld, int Np, int N, int S, double *__restrict__ part)
 {
-    const int slot = blockIdx.x, ch = blockIdx.y;
+    __shared__ double sh[256];
+    const int ch = blockIdx.x;
     const int r0 = (int)((long long)N * ch / RHO_CH), r1 = (int)((long long)N * (ch + 1) / RHO_CH);
-    double acc0 = 0.0, acc1 = 0.0;
-    for (int i = r0 + (threadIdx.x >> 5); i < r1; i += 8) {
-        const double *a = Astack + (size_t)i * ld + (size_t)slot * Np;
-        const double *pr = Pp + (size_t)i * Np;
-        int j = (threadIdx.x & 31) * 2;
-        for (; j + 1 < N; j += 64) {
-            const double2 av = *reinterpret_cast<const double2 *>(a + j);
-            const double2 pv = *reinterpret_cast<const double2 *>(pr + j);
-            acc0 = fma(pv.x, av.x, acc0);
-            acc1 = fma(pv.y, av.y, acc1);
+    const int ngrp = 256 / S, grp = threadIdx.x / S, slot = threadIdx.x % S;      // S <= 128
+    double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
+    if (grp < ngrp) {
+        for (int m = r0; m < r1; ++m) {
+            const double *a = Astack + (size_t)m * ld + slot;
+            const double *pr = Pp + (size_t)m * Np;
+            int n = grp;
+            for (; n + 3 * ngrp < N; n += 4 * ngrp) {
+                a0 = fma(pr[n], a[(size_t)n * S], a0);
+                a1 = fma(pr[n + ngrp], a[(size_t)(n + ngrp) * S], a1);
+                a2 = fma(pr[n + 2 * ngrp], a[(size_t)(n + 2 * ngrp) * S], a2);
+                a3 = fma(pr[n + 3 * ngrp], a[(size_t)(n + 3 * ngrp) * S], a3);
+            }
+            for (; n < N; n += ngrp) a0 = fma(pr[n], a[(size_t)n * S], a0);
         }
-        if (j < N) acc0 = fma(pr[j], a[j], acc0);
     }
-    double acc = acc0 + acc1;
-    __shared__ double s[8];
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
-    if ((threadIdx.x & 31) == 0) s[threadIdx.x >> 5] = acc;
+    sh[threadIdx.x] = (a0 + a1) + (a2 + a3);
     __syncthreads();
-    if (threadIdx.x == 0) {
+    if (threadIdx.x < S) {
         double t = 0.0;
-        for (int w = 0; w < 8; ++w) t += s[w];
-        part[slot * RHO_CH + ch] = t;
+        for (int g = 0; g < ngrp; ++g) t += sh[g * S + threadIdx.x];
+        part[(size_t)ch * S + threadIdx.x] = t;
     }
 }
-__global__ void rho_final_kernel(const double *__restrict__ part, int nslot, double *__restrict__ rho)
+__global__ void rho_final_kernel(const double *__restrict__ part, int S, double *__restrict__ rho)
 {
     const int slot = blockIdx.x * blockDim.x + threadIdx.x;
-    if (slot >= nslot) return;
+    if (slot >= S) return;
     double t = 0.0;
-    for (int c = 0; c < RHO_CH; ++c) t += part[slot * RHO_CH + c];
+    for (int c = 0; c < RHO_CH; ++c) t += part[(size_t)c * S + slot];
     rho[slot] = t;
 }
-int rho_scratch_doubles(int nslot) { return nslot * (RHO_CH + 1); }
-// rho: nslot results followed by nslot*RHO_CH partials (rho_scratch_doubles)
-void launch_rho_reduce(const double *Pp, const double *Astack, size_t ld, int Np, int N, int nslot, double *rho,
-                       cudaStream_t st)
+int rho_scratch_doubles(int S) { return S * (RHO_CH + 1); }
+// rho: S results followed by S*RHO_CH partials (rho_scratch_doubles)
+void launch_rho_reduce(const double *Pp, const double *Astack, int Np, int N, int S, double *rho, cudaStream_t st)
 {
-    if (nslot <= 0) return;
-    double *part = rho + nslot;
-    rho_reduce_kernel<<<dim3(nslot, RHO_CH), 256, 0, st>>>(Pp, Astack, ld, Np, N, part);
-    rho_final_kernel<<<(nslot + 127) / 128, 128, 0, st>>>(part, nslot, rho);
+    if (S <= 0) return;
+    double *part = rho + S;
+    rho_reduce_kernel<<<RHO_CH, 256, 0, st>>>(Pp, Astack, (size_t)Np * S, Np, N, S, part);
+    rho_final_kernel<<<(S + 127) / 128, 128, 0, st>>>(part, S, rho);
 }
 
-__global__ void jlr_accum_kernel(const double *__restrict__ Astack, size_t ld, int Np, int N, int nslot,
-                                 const double *__restrict__ rho, double sign, double *__restrict__ Jacc)
+// Jacc[m][n] += sign * sum_slot A'[m][n][slot] rho'[slot]: one warp per matrix element, lanes over the slots
+__global__ void __launch_bounds__(256) jlr_accum_kernel(const double *__restrict__ Astack, size_t ld, int N, int S,
+                                                        const double *__restrict__ rho, double sign, double *__restrict__ Jacc)
 {
-    const int n = blockIdx.x * blockDim.x + threadIdx.x, m = blockIdx.y;
-    if (n >= N) return;
-    const double *a = Astack + (size_t)m * ld + n;
-    double acc = 0.0;
-    for (int s = 0; s < nslot; ++s) acc = fma(a[(size_t)s * Np], rho[s], acc);
-    Jacc[(size_t)m * N + n] += sign * acc;
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    const int m = blockIdx.y;
+    double r[4];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) r[k] = lane + 32 * k < S ? rho[lane + 32 * k] : 0.0;
+    for (int n = blockIdx.x * 8 + w; n < N; n += gridDim.x * 8) {
+        const double *a = Astack + (size_t)m * ld + (size_t)n * S;
+        double acc = 0.0;
+#pragma unroll
+        for (int k = 0; k < 4; ++k)
+            if (lane + 32 * k < S) acc = fma(a[lane + 32 * k], r[k], acc);
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+        if (lane == 0) Jacc[(size_t)m * N + n] += sign * acc;
+    }
 }
-void launch_jlr_accum(const double *Astack, size_t ld, int Np, int N, int nslot, const double *rho, double sign,
-                      double *Jacc, cudaStream_t st)
+void launch_jlr_accum(const double *Astack, int Np, int N, int S, const double *rho, double sign, double *Jacc, cudaStream_t st)
 {
-    if (nslot <= 0) return;
-    dim3 grid((N + 127) / 128, N);
-    jlr_accum_kernel<<<grid, 128, 0, st>>>(Astack, ld, Np, N, nslot, rho, sign, Jacc);
+    if (S <= 0) return;
+    dim3 grid(8, N);
+    jlr_accum_kernel<<<grid, 256, 0, st>>>(Astack, (size_t)Np * S, N, S, rho, sign, Jacc);
 }
 
 // ---------------------------------------------------------------- FP64 tensor-core GEMM (A8, A9)
@@ -357,8 +384,10 @@ __device__ __forceinline__ void dmma(double &c0, double &c1, double a, double b)
 //   i.e. op(A) = A^T -- the Y^T Y form of the reciprocal-space K contraction.
 //   dyn (device, may be null): dyn[0] = rank r of the factor P' = L L^T (or N in the fallback), dyn[1] = use B_alt.
 //   use_dyn bit 0: only row tiles with bm*BM < r are computed; bit 1: Kb = roundup16(r); bit 2: B = B_alt if dyn[1];
+//   bit 3: nbatch = r (the batches are the rows of the factor);
 //   lower_only: tiles with bn > bm are skipped (symmetric result, completed in finalise).
-template <bool TA>
+//   TB = true: B_b is stored as Nc x Kb (k contiguous, ldb = row stride), i.e. C += op(A) B^T.
+template <bool TA, bool TB>
 __global__ void __launch_bounds__(256) dgemm_kernel(int Kb, int nbatch, double alpha, const double *__restrict__ A, size_t lda,
                                                     size_t strideA, const double *__restrict__ B, size_t ldb, size_t strideB,
                                                     double beta, double *__restrict__ C, size_t ldc, size_t strideC, int nsplit,
@@ -367,8 +396,9 @@ __global__ void __launch_bounds__(256) dgemm_kernel(int Kb, int nbatch, double a
 {
     extern __shared__ __align__(16) double smem[];
     constexpr int A_TILE = TA ? BK * SB : BM * SA;
+    constexpr int B_TILE = TB ? BN * SA : BK * SB;
     double *As = smem;                       // [2][A_TILE]
-    double *Bs = smem + 2 * A_TILE;          // [2][BK*SB]
+    double *Bs = smem + 2 * A_TILE;          // [2][B_TILE]
     const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
     const int wm = w >> 2, wn = w & 3;
     const int bm = blockIdx.y, bn = blockIdx.x, z = blockIdx.z;
@@ -378,6 +408,7 @@ __global__ void __launch_bounds__(256) dgemm_kernel(int Kb, int nbatch, double a
         if ((use_dyn & 1) && bm * BM >= r) return;
         if (use_dyn & 2) Kb = ((r + BK - 1) / BK) * BK;
         if ((use_dyn & 4) && dyn[1]) B = B_alt;
+        if (use_dyn & 8) nbatch = r;
     }
     const int bat0 = (int)((long long)nbatch * z / nsplit), bat1 = (int)((long long)nbatch * (z + 1) / nsplit);
     const int kt_per = Kb / BK;
@@ -392,8 +423,7 @@ __global__ void __launch_bounds__(256) dgemm_kernel(int Kb, int nbatch, double a
 
     auto load_tile = [&](int t, int buf) {
         const int b = bat0 + t / kt_per, k0 = (t % kt_per) * BK;
-        const double *Bb = B + (size_t)b * strideB + (size_t)k0 * ldb + bn * BN;
-        double *as = As + buf * A_TILE, *bs = Bs + buf * BK * SB;
+        double *as = As + buf * A_TILE, *bs = Bs + buf * B_TILE;
         if (TA) {
             const double *Ab = A + (size_t)b * strideA + (size_t)k0 * lda + bm * BM;
 #pragma unroll
@@ -409,10 +439,20 @@ __global__ void __launch_bounds__(256) dgemm_kernel(int Kb, int nbatch, double a
                 cp_async16(as + row * SA + c2 * 2, Ab + (size_t)row * lda + c2 * 2);
             }
         }
+        if (TB) {
+            const double *Bb = B + (size_t)b * strideB + (size_t)(bn * BN) * ldb + k0;
 #pragma unroll
-        for (int c = tid; c < BK * BN / 2; c += 256) {
-            const int row = c >> 6, c2 = c & 63;
-            cp_async16(bs + row * SB + c2 * 2, Bb + (size_t)row * ldb + c2 * 2);
+            for (int c = tid; c < BN * BK / 2; c += 256) {
+                const int row = c >> 3, c2 = c & 7;
+                cp_async16(bs + row * SA + c2 * 2, Bb + (size_t)row * ldb + c2 * 2);
+            }
+        } else {
+            const double *Bb = B + (size_t)b * strideB + (size_t)k0 * ldb + bn * BN;
+#pragma unroll
+            for (int c = tid; c < BK * BN / 2; c += 256) {
+                const int row = c >> 6, c2 = c & 63;
+                cp_async16(bs + row * SB + c2 * 2, Bb + (size_t)row * ldb + c2 * 2);
+            }
         }
         asm volatile("cp.async.commit_group;\n" ::);
     };
@@ -429,14 +469,15 @@ __global__ void __launch_bounds__(256) dgemm_kernel(int Kb, int nbatch, double a
         __syncthreads();
         const double *as = TA ? As + buf * A_TILE + (lane & 3) * SB + wm * 64 + (lane >> 2)
                               : As + buf * A_TILE + (wm * 64 + (lane >> 2)) * SA + (lane & 3);
-        const double *bs = Bs + buf * BK * SB + (lane & 3) * SB + wn * 32 + (lane >> 2);
+        const double *bs = TB ? Bs + buf * B_TILE + (wn * 32 + (lane >> 2)) * SA + (lane & 3)
+                              : Bs + buf * B_TILE + (lane & 3) * SB + wn * 32 + (lane >> 2);
 #pragma unroll
         for (int kk = 0; kk < BK; kk += 4) {
             double a[8], b[4];
 #pragma unroll
             for (int i = 0; i < 8; ++i) a[i] = TA ? as[kk * SB + i * 8] : as[i * 8 * SA + kk];
 #pragma unroll
-            for (int j = 0; j < 4; ++j) b[j] = bs[kk * SB + j * 8];
+            for (int j = 0; j < 4; ++j) b[j] = TB ? bs[j * 8 * SA + kk] : bs[kk * SB + j * 8];
 #pragma unroll
             for (int i = 0; i < 8; ++i)
 #pragma unroll
@@ -465,18 +506,26 @@ void launch_dgemm(const GemmArgs &g, cudaStream_t st)
 {
     static bool attr_set = false;
     constexpr int smemN = 2 * (BM * SA + BK * SB) * (int)sizeof(double), smemT = 2 * (2 * BK * SB) * (int)sizeof(double);
+    constexpr int smemNT = 2 * (BM * SA + BN * SA) * (int)sizeof(double);
     if (!attr_set) {
-        cudaFuncSetAttribute(dgemm_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smemN);
-        cudaFuncSetAttribute(dgemm_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smemT);
+        cudaFuncSetAttribute(dgemm_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smemN);
+        cudaFuncSetAttribute(dgemm_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smemT);
+        cudaFuncSetAttribute(dgemm_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smemNT);
         attr_set = true;
     }
     dim3 grid(g.Nc / BN, g.M / BM, g.nsplit);
     if (g.transA)
-        dgemm_kernel<true><<<grid, 256, smemT, st>>>(g.Kb, g.nbatch, g.alpha, g.A, g.lda, g.strideA, g.B, g.ldb, g.strideB, g.beta,
-                                                     g.C, g.ldc, g.strideC, g.nsplit, g.dyn, g.use_dyn, g.B_alt, g.lower_only);
+        dgemm_kernel<true, false><<<grid, 256, smemT, st>>>(g.Kb, g.nbatch, g.alpha, g.A, g.lda, g.strideA, g.B, g.ldb, g.strideB,
+                                                            g.beta, g.C, g.ldc, g.strideC, g.nsplit, g.dyn, g.use_dyn, g.B_alt,
+                                                            g.lower_only);
+    else if (g.transB)
+        dgemm_kernel<false, true><<<grid, 256, smemNT, st>>>(g.Kb, g.nbatch, g.alpha, g.A, g.lda, g.strideA, g.B, g.ldb, g.strideB,
+                                                             g.beta, g.C, g.ldc, g.strideC, g.nsplit, g.dyn, g.use_dyn, g.B_alt,
+                                                             g.lower_only);
     else
-        dgemm_kernel<false><<<grid, 256, smemN, st>>>(g.Kb, g.nbatch, g.alpha, g.A, g.lda, g.strideA, g.B, g.ldb, g.strideB, g.beta,
-                                                      g.C, g.ldc, g.strideC, g.nsplit, g.dyn, g.use_dyn, g.B_alt, g.lower_only);
+        dgemm_kernel<false, false><<<grid, 256, smemN, st>>>(g.Kb, g.nbatch, g.alpha, g.A, g.lda, g.strideA, g.B, g.ldb, g.strideB,
+                                                             g.beta, g.C, g.ldc, g.strideC, g.nsplit, g.dyn, g.use_dyn, g.B_alt,
+                                                             g.lower_only);
 }
 
 // ---------------------------------------------------------------- factor of P' for the K contraction (A8)
@@ -655,17 +704,17 @@ void launch_finalize_k(const double *Ksr, const ShellInfo &sh, const double *Klr
     finalize_k_kernel<<<grid, 128, 0, st>>>(Ksr, sh, Klr, nsplit, strideK, Np, N, fcomp, shell_of_ao, K);
 }
 
-__global__ void extract_overlap_kernel(const double *__restrict__ Astack, size_t ld, int N, const double *__restrict__ f,
-                                       double *__restrict__ S)
+__global__ void extract_overlap_kernel(const double *__restrict__ Astack, size_t ld, int S, int N, const double *__restrict__ f,
+                                       double *__restrict__ Sm)
 {
     const int n = blockIdx.x * blockDim.x + threadIdx.x, m = blockIdx.y;
     if (n >= N) return;
-    S[(size_t)m * N + n] = f[m] * f[n] * Astack[(size_t)m * ld + n];
+    Sm[(size_t)m * N + n] = f[m] * f[n] * Astack[(size_t)m * ld + (size_t)n * S];
 }
-void launch_extract_overlap(const double *Astack, size_t ld, int N, const double *fcomp, double *S, cudaStream_t st)
+void launch_extract_overlap(const double *Astack, int Np, int S, int N, const double *fcomp, double *Sm, cudaStream_t st)
 {
     dim3 grid((N + 127) / 128, N);
-    extract_overlap_kernel<<<grid, 128, 0, st>>>(Astack, ld, N, fcomp, S);
+    extract_overlap_kernel<<<grid, 128, 0, st>>>(Astack, (size_t)Np * S, S, N, fcomp, Sm);
 }
 
 // ---------------------------------------------------------------- FP64 FMA peak (roofline denominator)

@@ -12,6 +12,8 @@ struct LRParams {
     int N, Np;                 // basis size and its padded size (multiple of 128)
     const double *fcomp;       // [N] per-component factor (1 or sqrt 3)
     const double *Gx, *Gy, *Gz, *Gw;   // half-sphere G list, Gw = sqrt(2 * 4 pi/(Omega G^2) exp(-G^2/4w^2))
+    const int *sp_cls[9];      // shell pairs of U by class (l_A*3 + l_B): one agen_kernel instantiation each
+    int n_sp_cls[9];
 };
 
 // P' = f P f (into the padded Np x Np buffer, pads untouched) and ln(max |P'|)
@@ -25,17 +27,16 @@ void launch_hermite_density(const PairListU &U, const ShellInfo &sh, const KetLi
 // J_ab += sum_t (-1)^{|t|} E^{ab}_t Jt  per shell pair, mirrored (eq 96-97)
 void launch_j_backtransform(const PairListU &U, const ShellInfo &sh, const double *Jt, double *Jsr, int N,
                             cudaStream_t st);
-// A'(G) = sqrt(w) rho_mn(G) for G in [g0, g0+nb): real and imaginary parts as 2*nb slots of the
-// stack  A[row*ld + slot*Np + col], ld = 2*nb_alloc*Np.  g0 < 0: the single G = 0 slot with
-// weight `w0` (overlap S, eq 21), written to slot 0.
-void launch_agen(const LRParams &p, int g0, int nb, double w0, double *Astack, size_t ld, cudaStream_t st);
-// rho'[slot] = sum P' o A'[slot]; rho must hold rho_scratch_doubles(nslot) doubles (results, then partials)
-int rho_scratch_doubles(int nslot);
-void launch_rho_reduce(const double *Pp, const double *Astack, size_t ld, int Np, int N, int nslot, double *rho,
-                       cudaStream_t st);
-// Jacc[m][n] += sign * sum_slot A'[slot][m][n] rho'[slot]
-void launch_jlr_accum(const double *Astack, size_t ld, int Np, int N, int nslot, const double *rho, double sign,
-                      double *Jacc, cudaStream_t st);
+// A'(G) = sqrt(w) rho_mn(G) for G in [g0, g0+nb): real and imaginary parts as slots 2g, 2g+1 of the stack
+//   A'[row*ld + col*S + slot], ld = Np*S, S >= 2*nb a multiple of 16 (slots past 2*nb are written as 0).
+// g0 < 0: the single G = 0 slot with weight `w0` (overlap S, eq 21) in slot 0.
+void launch_agen(const LRParams &p, int g0, int nb, int S, double w0, double *Astack, cudaStream_t st);
+int agen_launches(const LRParams &p);
+// rho'[slot] = sum P' o A'[slot]; rho must hold rho_scratch_doubles(S) doubles (results, then partials)
+int rho_scratch_doubles(int S);
+void launch_rho_reduce(const double *Pp, const double *Astack, int Np, int N, int S, double *rho, cudaStream_t st);
+// Jacc[m][n] += sign * sum_slot A'[m][n][slot] rho'[slot]
+void launch_jlr_accum(const double *Astack, int Np, int N, int S, const double *rho, double sign, double *Jacc, cudaStream_t st);
 // C[z][M x Nc] (ldc) = beta*C + alpha * sum_b op(A_b)[M x Kb] B_b[Kb x Nc](ldb) over the batches of split z;
 // M, Nc multiples of 128, Kb of 16; grid.z = nsplit partial results C + z*strideC over disjoint batch ranges.
 // See dgemm_kernel in pbcjk_lr.cu for transA / dyn / lower_only.
@@ -47,7 +48,7 @@ struct GemmArgs {
     double beta = 0.0;
     double *C = nullptr; size_t ldc = 0, strideC = 0;
     int nsplit = 1;
-    bool transA = false;
+    bool transA = false, transB = false;
     const int *dyn = nullptr; int use_dyn = 0;
     const double *B_alt = nullptr;
     int lower_only = 0;
@@ -62,7 +63,7 @@ int factor_density_launches(int N);
 void launch_finalize_j(const double *Jsr, const double *Jlr, int N, const double *fcomp, double *J, cudaStream_t st);
 void launch_finalize_k(const double *Ksr, const ShellInfo &sh, const double *Klr, int nsplit, size_t strideK, int Np,
                        int N, const double *fcomp, const int *shell_of_ao, double *K, cudaStream_t st);
-void launch_extract_overlap(const double *Astack, size_t ld, int N, const double *fcomp, double *S, cudaStream_t st);
+void launch_extract_overlap(const double *Astack, int Np, int S, int N, const double *fcomp, double *Sm, cudaStream_t st);
 double run_fp64_peak(int iters);
 
 }  // namespace pbcjk
