@@ -573,7 +573,20 @@ int setup(pbc_jk *h, const pbc_cell *cell, const pbc_atoms *atoms, const pbc_she
         h->nb = nb;
         h->Smax = ((2 * nb + 15) / 16) * 16;             // slots of a full batch (multiple of 16)
         h->ld = (size_t)h->Smax * Np;
-        h->nsplit = Np <= 2048 ? 4 : 1;
+        // split of the K^LR accumulation over the rows of the factor: the lower 128x128 tiles times nsplit should
+        // fill whole waves of one CTA per SM
+        {
+            int nsm = 148;
+            cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, 0);
+            const long tiles = (long)(Np / 128) * (Np / 128 + 1) / 2;
+            double best = 0.0;
+            h->nsplit = 1;
+            for (int ns = 1; ns <= 8; ++ns) {
+                const long ctas = tiles * ns, waves = (ctas + nsm - 1) / nsm;
+                const double eff = (double)ctas / (double)(waves * nsm);
+                if (eff > best + 0.02) { best = eff; h->nsplit = ns; }
+            }
+        }
         CK(pool.alloc(&h->Pp, Np * Np)); CK(cudaMemset(h->Pp, 0, Np * Np * 8));
         CK(pool.alloc(&h->lnPmax, 1)); CK(pool.alloc(&h->maxbits, 1));
         CK(pool.alloc(&h->counters, CNT_N)); CK(cudaMemset(h->counters, 0, CNT_N * 8));
@@ -583,7 +596,7 @@ int setup(pbc_jk *h, const pbc_cell *cell, const pbc_atoms *atoms, const pbc_she
         CK(pool.alloc(&h->Klr, (size_t)h->nsplit * Np * Np));
         CK(pool.alloc(&h->Astack, Np * h->ld)); CK(cudaMemset(h->Astack, 0, Np * h->ld * 8));
         CK(pool.alloc(&h->Zstack, Np * h->ld));
-        CK(pool.alloc(&h->rho, (size_t)rho_scratch_doubles(h->Smax)));
+        CK(pool.alloc(&h->rho, (size_t)rho_scratch_doubles(h->Smax, nbf)));
         CK(pool.alloc(&h->LT, Np * Np)); CK(pool.alloc(&h->chol_d, 2 * Np)); CK(pool.alloc(&h->chol_s, 2));
         CK(pool.alloc(&h->chol_dyn, 4));
         CK(pool.alloc(&h->hostP, N * N)); CK(pool.alloc(&h->hostJ, N * N)); CK(pool.alloc(&h->hostK, N * N));

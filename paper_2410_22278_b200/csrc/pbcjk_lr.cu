@@ -282,55 +282,59 @@ void launch_agen(const LRParams &p, int g0, int nb, int S, double w0, double *As
     launch_agen_class<2, 2>(p, g0, nb, S, w0, Astack, ld, st);
 }
 
-// rho'[slot] = sum_{mn} P'_mn A'_mn[slot]: RHO_CH row chunks, threads over the (contiguous) slots, then a
-// fixed-order sum of the chunk partials (deterministic).  HBM-bound: streams the stored batch once.
-constexpr int RHO_CH = 296;
+// rho'[slot] = sum_{mn} P'_mn A'_mn[slot]: one block per row m, threads over the (contiguous) slots and groups of
+// columns, then a fixed-order sum of the row partials (deterministic).  HBM-bound: streams the stored batch once.
 __global__ void __launch_bounds__(256) rho_reduce_kernel(const double *__restrict__ Pp, const double *__restrict__ Astack,
                                                          size_t ld, int Np, int N, int S, double *__restrict__ part)
 {
     __shared__ double sh[256];
-    const int ch = blockIdx.x;
-    const int r0 = (int)((long long)N * ch / RHO_CH), r1 = (int)((long long)N * (ch + 1) / RHO_CH);
+    const int m = blockIdx.x;
     const int ngrp = 256 / S, grp = threadIdx.x / S, slot = threadIdx.x % S;      // S <= 128
     double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
     if (grp < ngrp) {
-        for (int m = r0; m < r1; ++m) {
-            const double *a = Astack + (size_t)m * ld + slot;
-            const double *pr = Pp + (size_t)m * Np;
-            int n = grp;
-            for (; n + 3 * ngrp < N; n += 4 * ngrp) {
-                a0 = fma(pr[n], a[(size_t)n * S], a0);
-                a1 = fma(pr[n + ngrp], a[(size_t)(n + ngrp) * S], a1);
-                a2 = fma(pr[n + 2 * ngrp], a[(size_t)(n + 2 * ngrp) * S], a2);
-                a3 = fma(pr[n + 3 * ngrp], a[(size_t)(n + 3 * ngrp) * S], a3);
-            }
-            for (; n < N; n += ngrp) a0 = fma(pr[n], a[(size_t)n * S], a0);
+        const double *a = Astack + (size_t)m * ld + slot;
+        const double *pr = Pp + (size_t)m * Np;
+        int n = grp;
+        for (; n + 3 * ngrp < N; n += 4 * ngrp) {
+            a0 = fma(pr[n], a[(size_t)n * S], a0);
+            a1 = fma(pr[n + ngrp], a[(size_t)(n + ngrp) * S], a1);
+            a2 = fma(pr[n + 2 * ngrp], a[(size_t)(n + 2 * ngrp) * S], a2);
+            a3 = fma(pr[n + 3 * ngrp], a[(size_t)(n + 3 * ngrp) * S], a3);
         }
+        for (; n < N; n += ngrp) a0 = fma(pr[n], a[(size_t)n * S], a0);
     }
     sh[threadIdx.x] = (a0 + a1) + (a2 + a3);
     __syncthreads();
     if (threadIdx.x < S) {
         double t = 0.0;
         for (int g = 0; g < ngrp; ++g) t += sh[g * S + threadIdx.x];
-        part[(size_t)ch * S + threadIdx.x] = t;
+        part[(size_t)m * S + threadIdx.x] = t;
     }
 }
-__global__ void rho_final_kernel(const double *__restrict__ part, int S, double *__restrict__ rho)
+// rho[slot] = sum_m part[m][slot]: 8 row groups per slot, summed in a fixed order
+__global__ void __launch_bounds__(1024) rho_final_kernel(const double *__restrict__ part, int N, int S, double *__restrict__ rho)
 {
-    const int slot = blockIdx.x * blockDim.x + threadIdx.x;
-    if (slot >= S) return;
+    __shared__ double sh[1024];
+    const int slot = threadIdx.x % 128, grp = threadIdx.x / 128;
     double t = 0.0;
-    for (int c = 0; c < RHO_CH; ++c) t += part[(size_t)c * S + slot];
-    rho[slot] = t;
+    if (slot < S)
+        for (int m = grp; m < N; m += 8) t += part[(size_t)m * S + slot];
+    sh[threadIdx.x] = t;
+    __syncthreads();
+    if (threadIdx.x < S) {
+        double r = 0.0;
+        for (int g = 0; g < 8; ++g) r += sh[g * 128 + threadIdx.x];
+        rho[threadIdx.x] = r;
+    }
 }
-int rho_scratch_doubles(int S) { return S * (RHO_CH + 1); }
-// rho: S results followed by S*RHO_CH partials (rho_scratch_doubles)
+int rho_scratch_doubles(int S, int N) { return S * (N + 1); }
+// rho: S results followed by S*N row partials (rho_scratch_doubles)
 void launch_rho_reduce(const double *Pp, const double *Astack, int Np, int N, int S, double *rho, cudaStream_t st)
 {
     if (S <= 0) return;
     double *part = rho + S;
-    rho_reduce_kernel<<<RHO_CH, 256, 0, st>>>(Pp, Astack, (size_t)Np * S, Np, N, S, part);
-    rho_final_kernel<<<(S + 127) / 128, 128, 0, st>>>(part, S, rho);
+    rho_reduce_kernel<<<N, 256, 0, st>>>(Pp, Astack, (size_t)Np * S, Np, N, S, part);
+    rho_final_kernel<<<1, 1024, 0, st>>>(part, N, S, rho);
 }
 
 // Jacc[m][n] += sign * sum_slot A'[m][n][slot] rho'[slot]: one warp per matrix element, lanes over the slots

@@ -32,8 +32,8 @@ void launch_j_backtransform(const PairListU &U, const ShellInfo &sh, const doubl
 // g0 < 0: the single G = 0 slot with weight `w0` (overlap S, eq 21) in slot 0.
 void launch_agen(const LRParams &p, int g0, int nb, int S, double w0, double *Astack, cudaStream_t st);
 int agen_launches(const LRParams &p);
-// rho'[slot] = sum P' o A'[slot]; rho must hold rho_scratch_doubles(S) doubles (results, then partials)
-int rho_scratch_doubles(int S);
+// rho'[slot] = sum P' o A'[slot]; rho must hold rho_scratch_doubles(S, N) doubles (results, then row partials)
+int rho_scratch_doubles(int S, int N);
 void launch_rho_reduce(const double *Pp, const double *Astack, int Np, int N, int S, double *rho, cudaStream_t st);
 // Jacc[m][n] += sign * sum_slot A'[m][n][slot] rho'[slot]
 void launch_jlr_accum(const double *Astack, int Np, int N, int S, const double *rho, double sign, double *Jacc, cudaStream_t st);
