@@ -138,6 +138,25 @@ def _peaks():
     return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "sm_max_mhz": 1965.0}, "fallback"
 
 
+def _ncu_traffic(kernel):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel` from the committed ncu --set full capture
+    (profiles/r1_ncu_traffic.json, written by hand from the capture named there); None when it holds no such kernel."""
+    p = os.path.join(ROOT, "profiles", "r1_ncu_traffic.json")
+    if not os.path.exists(p):
+        return None
+    return json.load(open(p)).get("dram_bytes_per_launch", {}).get(kernel)
+
+
+def _lr_roofline(st, n, rank, peak_tf):
+    slots = 2 * st["n_g"] + 1                       # Re and Im of every G of the half sphere, plus the SELF slot
+    flop = (2.0 * rank * n * n + rank * n * (n + 1.0)) * slots
+    ms = st["ms_lr"]
+    tf = flop / (ms * 1e-3) * 1e-12 if ms > 0 else 0.0
+    return {"ms": ms, "bound": "tensor (FP64 DMMA, mma.sync.m8n8k4.f64)", "gemm_flop": flop, "rank_of_P": rank,
+            "tflops_over_whole_phase": tf, "frac_of_fp64_peak": tf / peak_tf,
+            "note": "the phase time also holds rho_mn(G) generation, the rho(G)/J^LR passes (HBM-bound) and the Cholesky factor of P"}
+
+
 def _oracle_sample_blocks(wl, nblk, seed=12345):
     """Seeded sample of output shell blocks covering every (l_mu, l_nu) class of the workload."""
     rng = np.random.default_rng(seed)
@@ -224,7 +243,8 @@ def main():
     ap.add_argument("--workload", default="water64",
                     help="tiny | water8 | si64 | water64 (config 4, the 192-atom metric config) | water343")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--precision", default="fp64", choices=["fp64", "mixed"])
+    ap.add_argument("--precision", default="fp64", choices=["fp64"],
+                    help="mixed precision (PAPER 3.5) is not built yet; pbc_jk_create refuses it")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
@@ -341,13 +361,16 @@ def main():
             "achieved": top_tf, "peak": fp64_nominal, "unit": "TFLOP/s", "frac": top_tf / fp64_nominal,
             "peak_kind": f"FP64 FMA: 148 SM x 64 lanes x 2 x {sm_max:.0f} MHz (DESIGN.md); DFMA micro-benchmark on this box: "
                          f"{fp64_meas:.2f} TFLOP/s",
-            "traffic": None,
+            "traffic": _ncu_traffic(f"sr_{top['kind'].lower()}_kernel<{','.join(map(str, top['l']))}>"),
             "flop_per_quartet": class_flops(top), "quartets_per_launch": top["quartets"], "ms_per_launch": top["ms"],
             "share_of_step": top["ms"] / ms_per_step,
             "real_space_all_classes": {"ms": sr_ms, "tflops": sr_flop / (sr_ms * 1e-3) * 1e-12 if sr_ms > 0 else 0.0,
                                        "frac": (sr_flop / (sr_ms * 1e-3) * 1e-12 / fp64_nominal) if sr_ms > 0 else 0.0},
             "families": {k: {"ms": v["ms"], "quartets": v["quartets"],
                              "tflops": v["flop"] / (v["ms"] * 1e-3) * 1e-12 if v["ms"] > 0 else 0.0} for k, v in fam.items()},
+            # reciprocal-space phase (A7-A9): its dense part is two FP64 tensor-core GEMMs per G batch,
+            # Y = L^T A' (2 r N^2 flop per slot) and K += Y^T Y on the lower triangle (r N (N+1) flop per slot)
+            "reciprocal_space": _lr_roofline(st, n, wl.n_occ, fp64_nominal),
             "top_classes": [{"kind": c["kind"], "l": list(c["l"]), "ms": round(c["ms"], 3), "quartets": c["quartets"],
                              "tflops": round(class_flops(c) * c["quartets"] / (c["ms"] * 1e-3) * 1e-12, 3) if c["ms"] > 0 else 0.0}
                             for c in rows[:8]],

@@ -41,7 +41,8 @@ typedef enum {
     PBC_JK_ERR_INVALID_ARG = -1,   /* null pointer, w <= 0, singular cell, l > 2, exponent <= 0, nprim < 1 */
     PBC_JK_ERR_NOMEM = -2,         /* host or device allocation failed */
     PBC_JK_ERR_CUDA = -3,          /* CUDA runtime error; text via pbc_jk_last_error */
-    PBC_JK_ERR_UNSUPPORTED = -4    /* image index range exceeds the packed format (cell far too small) */
+    PBC_JK_ERR_UNSUPPORTED = -4    /* image index range exceeds the packed format (cell far too small), or      */
+                                   /* precision = 1 (mixed precision is not built yet: fp64 only)                */
 } pbc_jk_status;
 
 typedef struct pbc_jk pbc_jk;      /* opaque handle: owns all host + device state of one geometry */
@@ -69,10 +70,11 @@ typedef struct {
     double d_schwarz;    /* primitive quartet-image evaluated iff bound_bra*bound_ket*max|P|*          */
                          /* exp(-alpha_w r^2) (eq 67) exceeds this; default 1e-13                 */
     double d_ewald_k;    /* sets the default g_cut; default 1e-14                                      */
-    int32_t precision;   /* 0 = fp64 everywhere; 1 = mixed (PAPER 3.5 L817-821): quartets whose       */
-                         /* density-weighted bound is below mixed_switch run in fp32, fp64 accumulate  */
-    double mixed_switch; /* default 1e-5 (L819)                                                        */
-    int32_t lr_g_batch;  /* G vectors per reciprocal-space batch (0: sized from free memory)           */
+    int32_t precision;   /* 0 = fp64 everywhere.  1 = mixed (PAPER 3.5 L817-821: quartets whose       */
+                         /* density-weighted bound is below mixed_switch in fp32, fp64 accumulation)   */
+                         /* is NOT built yet: pbc_jk_create returns PBC_JK_ERR_UNSUPPORTED for it      */
+    double mixed_switch; /* reserved for precision = 1; default 1e-5 (L819)                            */
+    int32_t lr_g_batch;  /* G vectors per reciprocal-space batch (0: sized to <= 12 GB per stack; <=64)*/
 } pbc_cutoffs;
 
 /* Counters and phase times of the LAST pbc_jk_build (times need pbc_jk_sync_stats). */

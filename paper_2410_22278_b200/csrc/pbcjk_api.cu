@@ -635,6 +635,8 @@ int pbc_jk_create(const pbc_cell *cell, const pbc_atoms *atoms, const pbc_shells
         cudaGetLastError();
         return fail(nullptr, PBC_JK_ERR_CUDA, "no CUDA device: libpbc_jk has no CPU fallback");
     }
+    if (cut && cut->precision != 0)
+        return fail(nullptr, PBC_JK_ERR_UNSUPPORTED, "precision = 1 (mixed fp32/fp64 quartets) is not implemented: fp64 only");
     pbc_jk *h = new (std::nothrow) pbc_jk();
     if (!h) return fail(nullptr, PBC_JK_ERR_NOMEM, "host allocation failed");
     if (cut) h->cut = *cut;
