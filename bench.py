@@ -173,7 +173,7 @@ def _oracle_sample_blocks(wl, nblk, seed=12345):
     return blocks
 
 
-def _time_oracle(wl, P, target_s=15.0, max_blocks=64):
+def _time_oracle(wl, P, target_s=15.0, max_blocks=256):
     """The oracle as it stands on a bounded sample: its real-space (SR) part -- the part the metric's
     quartets belong to -- for a growing number of sampled output shell blocks until ~target_s of wall
     time was spent.  (The oracle's reciprocal-space pass costs the same for one block as for all of
