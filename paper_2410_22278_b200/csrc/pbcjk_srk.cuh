@@ -17,12 +17,14 @@ namespace pbcjk {
 
 template <int LA, int LB, int LC, int LD> struct KEval;      // specialisations: build/gen/k_eval_*.cuh
 
-__host__ __device__ constexpr int k_nthreads(int L) { return L >= 7 ? 64 : 128; }
+// CTA size: the R columns of a thread take 8*nherm(L) bytes of shared memory (672 B at L = 6, 1320 B at L = 8), so
+// high classes use 64-thread CTAs -- several small CTAs per SM keep more warps resident than one large one.
+__host__ __device__ constexpr int k_nthreads(int L) { return L >= 6 ? 64 : 128; }
 
 // bra slots per warp: a queued quartet refers to its bra by slot, so the queue carries survivors across bras
 // and the evaluator runs with (nearly) all 32 lanes; the slot stride is odd so that lanes reading the E tables
 // of different slots hit different banks.
-__host__ __device__ constexpr int k_nslot(int nterm) { return nterm > 150 ? 4 : 8; }
+__host__ __device__ constexpr int k_nslot(int nterm, int L) { return L >= 7 ? 2 : (nterm > 150 ? 4 : 8); }
 __host__ __device__ constexpr int k_slot_stride(int nterm) { return (nterm + 6) | 1; }   // E row + 6 scalars, odd
 constexpr int KQ = 64;                                       // ring capacity per warp (power of two)
 
@@ -31,7 +33,7 @@ constexpr size_t k_smem_bytes()
 {
     constexpr int L = LA + LB + LC + LD, NT = k_nthreads(L), NW = NT / 32;
     constexpr int NTERM = bra_terms<LA, LB>();
-    size_t d = (L > 4 ? (size_t)nherm(L) * NT : 0) + (size_t)NW * k_nslot(NTERM) * k_slot_stride(NTERM) +
+    size_t d = (L > 4 ? (size_t)nherm(L) * NT : 0) + (size_t)NW * k_nslot(NTERM, L) * k_slot_stride(NTERM) +
                (size_t)NW * ncart(LA) * ncart(LD);
     return d * sizeof(double) + (size_t)NW * KQ * (sizeof(int2) + sizeof(int));
 }
@@ -44,7 +46,7 @@ sr_k_kernel(SRParams p, const int2 *__restrict__ blocks, int nblocks)
     constexpr int NT = k_nthreads(L), NW = NT / 32;
     constexpr int NA = ncart(LA), ND = ncart(LD);
     constexpr int NTERM = bra_terms<LA, LB>();
-    constexpr int NSLOT = k_nslot(NTERM), SSTR = k_slot_stride(NTERM);
+    constexpr int NSLOT = k_nslot(NTERM, L), SSTR = k_slot_stride(NTERM);
     constexpr bool RSMEM = L > 4;
     using Ev = KEval<LA, LB, LC, LD>;
     static_assert(Ev::NBRA == NTERM, "generator and kernel disagree on the bra table");
