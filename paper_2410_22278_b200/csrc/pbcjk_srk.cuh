@@ -17,14 +17,14 @@ namespace pbcjk {
 
 template <int LA, int LB, int LC, int LD> struct KEval;      // specialisations: build/gen/k_eval_*.cuh
 
-// CTA size: the R columns of a thread take 8*nherm(L) bytes of shared memory (672 B at L = 6, 1320 B at L = 8), so
-// high classes use 64-thread CTAs -- several small CTAs per SM keep more warps resident than one large one.
-__host__ __device__ constexpr int k_nthreads(int L) { return L >= 6 ? 64 : 128; }
+// CTA size: the R column of a thread takes 8*nherm(L) bytes of shared memory (672 B at L = 6, 1320 B at L = 8);
+// 64-thread CTAs from L = 7 (measured: 64 threads already at L = 6, or 2 bra slots at L >= 7, is 5 % slower).
+__host__ __device__ constexpr int k_nthreads(int L) { return L >= 7 ? 64 : 128; }
 
 // bra slots per warp: a queued quartet refers to its bra by slot, so the queue carries survivors across bras
 // and the evaluator runs with (nearly) all 32 lanes; the slot stride is odd so that lanes reading the E tables
 // of different slots hit different banks.
-__host__ __device__ constexpr int k_nslot(int nterm, int L) { return L >= 7 ? 2 : (nterm > 150 ? 4 : 8); }
+__host__ __device__ constexpr int k_nslot(int nterm, int) { return nterm > 150 ? 4 : 8; }
 __host__ __device__ constexpr int k_slot_stride(int nterm) { return (nterm + 6) | 1; }   // E row + 6 scalars, odd
 constexpr int KQ = 64;                                       // ring capacity per warp (power of two)
 
