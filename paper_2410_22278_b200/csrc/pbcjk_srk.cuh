@@ -38,8 +38,11 @@ constexpr size_t k_smem_bytes()
     return d * sizeof(double) + (size_t)NW * KQ * (sizeof(int2) + sizeof(int));
 }
 
+// light classes: at most 128 registers so that 4 CTAs (16 warps) stay resident per SM
+__host__ __device__ constexpr int k_minblocks(int L) { return L <= 3 ? 4 : 1; }
+
 template <int LA, int LB, int LC, int LD>
-__global__ void __launch_bounds__(k_nthreads(LA + LB + LC + LD))
+__global__ void __launch_bounds__(k_nthreads(LA + LB + LC + LD), k_minblocks(LA + LB + LC + LD))
 sr_k_kernel(SRParams p, const int2 *__restrict__ blocks, int nblocks)
 {
     constexpr int L = LA + LB + LC + LD;
