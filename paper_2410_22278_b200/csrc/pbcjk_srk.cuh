@@ -51,6 +51,7 @@ sr_k_kernel(SRParams p, const int2 *__restrict__ blocks, int nblocks)
     constexpr int NTERM = bra_terms<LA, LB>();
     constexpr int NSLOT = k_nslot(NTERM, L), SSTR = k_slot_stride(NTERM);
     constexpr bool RSMEM = L > 4;
+    constexpr bool LOCKSTEP = L >= 5;
     using Ev = KEval<LA, LB, LC, LD>;
     static_assert(Ev::NBRA == NTERM, "generator and kernel disagree on the bra table");
     extern __shared__ __align__(16) double smem[];
@@ -197,7 +198,14 @@ sr_k_kernel(SRParams p, const int2 *__restrict__ blocks, int nblocks)
             j0 += 32;
             __syncwarp();
         }
-        if (qn == 0) break;                                           // nothing queued and no bra left
+        if (LOCKSTEP) {
+            // the evaluators of the high classes are 10-60 thousand instructions of straight-line code, far more than
+            // the instruction caches hold (ncu: 45 % of the stall samples of (dp|dp) were "no instruction"); the warps
+            // of a CTA therefore enter the evaluator together and share the fetched lines.  Every warp passes this
+            // barrier once per round until no warp has anything queued.
+            if (!__syncthreads_or(qn > 0)) break;
+            if (qn == 0) continue;
+        } else if (qn == 0) break;                                    // nothing queued and no bra left
         // ---- phase 2: one primitive quartet-image per lane, oldest survivors first ----
         const int take = qn < 32 ? qn : 32;
         if (lane < take) {
