@@ -17,9 +17,11 @@ namespace pbcjk {
 
 template <int LA, int LB, int LC, int LD> struct KEval;      // specialisations: build/gen/k_eval_*.cuh
 
-// CTA size: the R column of a thread takes 8*nherm(L) bytes of shared memory (672 B at L = 6, 1320 B at L = 8);
-// 64-thread CTAs from L = 7 (measured: 64 threads already at L = 6, or 2 bra slots at L >= 7, is 5 % slower).
-__host__ __device__ constexpr int k_nthreads(int L) { return L >= 7 ? 64 : 128; }
+// CTA size: 128 threads in every class.  The warps of a CTA enter the evaluator in lockstep at L >= 5 (see LOCKSTEP
+// below), so four warps share the instruction fetches; the R column of a thread takes 8*nherm(L) bytes of shared
+// memory (1320 B at L = 8: one CTA per SM).  Measured on water64 / si64: 64-thread CTAs at L >= 7 are 3 % slower,
+// 256-thread CTAs at L = 5 are 4-6 % slower, lockstep at L = 3, 4 is 10 % slower.
+__host__ __device__ constexpr int k_nthreads(int) { return 128; }
 
 // bra slots per warp: a queued quartet refers to its bra by slot, so the queue carries survivors across bras
 // and the evaluator runs with (nearly) all 32 lanes; the slot stride is odd so that lanes reading the E tables
