@@ -104,8 +104,9 @@ typedef struct {
 /*
  * A1-A3: validates, builds the reciprocal lattice and the half-sphere G list
  * (eq 32-36), the image-summed primitive pair lists with bounds (Fig 1, eq 57-61
- * L449-469, lattice enumeration eq 99-103), the Boys tables, and the crystalline overlap
- * S (eq 21); uploads everything; sizes all workspaces.  `cut` may be NULL (all defaults).
+ * L449-469, lattice enumeration eq 99-103), the Hermite expansion coefficient products
+ * E^{ab}_t of every primitive pair-image (eq 16-20), the Boys tables, and the crystalline
+ * overlap S (eq 21); uploads everything; sizes all workspaces.  `cut` may be NULL (all defaults).
  * Uses the current CUDA device.  On failure *out is NULL.
  */
 int pbc_jk_create(const pbc_cell *cell, const pbc_atoms *atoms, const pbc_shells *shells,
