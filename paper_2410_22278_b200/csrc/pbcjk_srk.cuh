@@ -40,8 +40,9 @@ constexpr size_t k_smem_bytes()
     return d * sizeof(double) + (size_t)NW * KQ * (sizeof(int2) + sizeof(int));
 }
 
-// light classes: at most 128 registers so that 4 CTAs (16 warps) stay resident per SM
-__host__ __device__ constexpr int k_minblocks(int L) { return L <= 3 ? 4 : 1; }
+// light classes: at most 128 registers (L <= 3: 4 CTAs, 16 warps per SM) or 168 (L = 4: 3 CTAs); the few spilled
+// doubles (<= 300 B per thread) cost less than the lost occupancy
+__host__ __device__ constexpr int k_minblocks(int L) { return L <= 3 ? 4 : (L == 4 ? 3 : 1); }
 
 template <int LA, int LB, int LC, int LD>
 __global__ void __launch_bounds__(k_nthreads(LA + LB + LC + LD), k_minblocks(LA + LB + LC + LD))
