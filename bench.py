@@ -12,8 +12,11 @@ separately.  Rank 0 prints ONE JSON line:
            J+K build time itself.
   value    device-resident leg: P, J, K live in HBM; CUDA events on the build's stream.
   e2e      same through pbc_jk_build_host with pinned HOST buffers (P up, J and K down, per step).
-  roofline dominant real-space kernel class against the FP64 FMA peak.
-  cpu_baseline  the fp64 oracle, as it stands, on a bounded sample of output shell blocks.
+  roofline the kernel family with the largest share of the step -- the reciprocal-space K GEMMs (FP64 tensor
+           cores, DMMA) or the real-space quartet kernels (FP64 FMA pipe) -- with both families printed
+           (DESIGN.md section 7); peaks measured live by the helper library libpbc_jk_benchpeaks.so.
+  cpu_baseline  the fp64 oracle, as it stands, on a bounded sample of output shell blocks, and the
+           extrapolation of that sample to a full build.
 
 --impl reference times the oracle alone (the reference arm of this tier).
 """
@@ -139,22 +142,23 @@ def _peaks():
 
 
 def _ncu_traffic(kernel):
-    """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel` from the committed ncu --set full capture
-    (profiles/r1_ncu_traffic.json, written by hand from the capture named there); None when it holds no such kernel."""
-    p = os.path.join(ROOT, "profiles", "r1_ncu_traffic.json")
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel` from the committed raw-page CSV extract of an
+    `ncu --set full` capture (profiles/r2_ncu_dram_bytes.csv: kernel, launches, bytes_read, bytes_write; written by the
+    command named in profiles/r2_ncu_dram_bytes.md).  None (= not measured) when the file or the kernel is absent."""
+    p = os.path.join(ROOT, "profiles", "r2_ncu_dram_bytes.csv")
     if not os.path.exists(p):
         return None
-    return json.load(open(p)).get("dram_bytes_per_launch", {}).get(kernel)
+    import csv
+    for row in csv.DictReader(open(p)):
+        if row["kernel"] == kernel:
+            return (float(row["bytes_read"]) + float(row["bytes_write"])) / max(1.0, float(row["launches"]))
+    return None
 
 
-def _lr_roofline(st, n, rank, peak_tf):
-    slots = 2 * st["n_g"] + 1                       # Re and Im of every G of the half sphere, plus the SELF slot
-    flop = (2.0 * rank * n * n + rank * n * (n + 1.0)) * slots
-    ms = st["ms_lr"]
-    tf = flop / (ms * 1e-3) * 1e-12 if ms > 0 else 0.0
-    return {"ms": ms, "bound": "tensor (FP64 DMMA, mma.sync.m8n8k4.f64)", "gemm_flop": flop, "rank_of_P": rank,
-            "tflops_over_whole_phase": tf, "frac_of_fp64_peak": tf / peak_tf,
-            "note": "the phase time also holds rho_mn(G) generation, the rho(G)/J^LR passes (HBM-bound) and the Cholesky factor of P"}
+def h_nb(st, n):
+    """G vectors per reciprocal-space batch as pbc_jk_create sizes them (stacks <= 12 GB, at most 64)"""
+    np_ = ((n + 127) // 128) * 128
+    return max(1, min(64, int(12.0e9 // (np_ * np_ * 16)), max(st["n_g"], 1)))
 
 
 def _oracle_sample_blocks(wl, nblk, seed=12345):
@@ -193,6 +197,37 @@ def _time_oracle(wl, P, target_s=15.0, max_blocks=256):
             break
         nblk = min(max_blocks, max(nblk + 1, int(nblk * min(8.0, 0.8 * target_s / max(dt, 1e-3)))))
     return q, dt, nblk, cores
+
+
+def _extrapolate_oracle(wl, P, nblk, n_g_half):
+    """the sampled oracle times extrapolated to a full build, labelled as such.  Real space: the sample is
+    stratified by output class (l_mu >= l_nu), so each class is timed on its own sampled blocks and scaled by the number
+    of ordered output blocks of that class.  Reciprocal space: the oracle's G pass costs the same for one block as for
+    all (it rebuilds rho_mn(G) of every pair per G), so a short window of G is timed and scaled by the G count."""
+    import oracle
+    blocks = _oracle_sample_blocks(wl, nblk)
+    ls = [int(l) for l in wl.sh_l]
+    cnt_l = {l: ls.count(l) for l in set(ls)}
+    per_class = {}
+    for (a, b) in blocks:
+        per_class.setdefault((ls[a], ls[b]), []).append((a, b))
+    sr_full = 0.0
+    for (la, lb), blk in per_class.items():
+        t0 = time.perf_counter()
+        oracle.jk(wl, P, blocks=blk, parts="sr")
+        dt = time.perf_counter() - t0
+        n_ordered = cnt_l[la] * cnt_l[lb] * (1 if la == lb else 2)
+        sr_full += dt / len(blk) * n_ordered
+    # G window: |G| up to about 2.4 reciprocal-lattice spacings (a few dozen vectors)
+    g_win = 2.4 * 2.0 * np.pi / float(np.linalg.norm(wl.cell, axis=1).max())
+    t0 = time.perf_counter()
+    r = oracle.jk(wl, P, blocks=blocks[:1], parts="lr", g_cut=g_win)
+    dt = time.perf_counter() - t0
+    ng = max(1, r["counts"]["n_G"])
+    lr_full = dt / ng * (2 * n_g_half)
+    return {"extrapolated_full_build_seconds": sr_full + lr_full,
+            "extrapolation": f"EXTRAPOLATED: real space {sr_full:.0f} s (per-class sampled seconds x ordered blocks of the class), "
+                             f"reciprocal space {lr_full:.0f} s ({dt / ng:.3f} s per G over {ng} G x {2 * n_g_half} G of the full sphere)"}
 
 
 def _workload_and_density(name):
@@ -243,8 +278,8 @@ def main():
     ap.add_argument("--workload", default="water64",
                     help="tiny | water8 | si64 | water64 (config 4, the 192-atom metric config) | water343")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--precision", default="fp64", choices=["fp64"],
-                    help="mixed precision (PAPER 3.5) is not built yet; pbc_jk_create refuses it")
+    ap.add_argument("--precision", default="fp64", choices=["fp64", "mixed"],
+                    help="mixed: real-space K quartets below the switch in fp32 (PAPER 3.5 L817-821)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
@@ -260,7 +295,7 @@ def main():
     import torch
     import torch.distributed as dist
     from paper_2410_22278_b200 import workloads
-    from paper_2410_22278_b200.binding import PbcJK, fp64_peak_tflops, load
+    from paper_2410_22278_b200.binding import PbcJK, allreduce_jk, bench_peaks, load
 
     load()                                             # fails loudly if libpbc_jk.so is missing
     if not torch.cuda.is_available():
@@ -274,10 +309,14 @@ def main():
     n = h.nbf
     S = h.overlap()                                    # the library's own crystalline overlap (A3)
     P = workloads.density_from_orbitals(wl.orbitals_seed(), S)
+    # N > 1: ONE build sharded over the ranks (real-space blocks / bras and G batches dealt round-robin),
+    # partial matrices summed by one all-reduce of [J; K] -- total work fixed: strong scaling
+    if world > 1:
+        h.set_shard(rank, world)
 
     Pd = torch.from_numpy(P).cuda()
-    Jd = torch.empty_like(Pd)
-    Kd = torch.empty_like(Pd)
+    JK = torch.empty((2, n, n), dtype=torch.float64, device="cuda")      # J and K back to back: one all-reduce message
+    Jd, Kd = JK[0], JK[1]
     Ph = torch.from_numpy(P).pin_memory()
     Jh = torch.empty((n, n), dtype=torch.float64).pin_memory()
     Kh = torch.empty((n, n), dtype=torch.float64).pin_memory()
@@ -289,92 +328,127 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
-    h.set_profile(True)
+    def step():
+        h.build(Pd, Jd, Kd)
+        if world > 1:
+            allreduce_jk(Jd, Kd)
+
+    h.set_profile(True)                                # an event pair per class launch and per GEMM pair: the roofline times
     # ---------------- device-resident leg ----------------
     for _ in range(args.warmup):
         flush.zero_()
-        h.build(Pd, Jd, Kd)
+        step()
     barrier()
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
     cls_ms = {}
+    gemm_ms = 0.0
     with ClockSampler(local_rank) as clocks:
         barrier()
         for i in range(args.steps):
             flush.zero_()                              # L2 flush between timed iterations (outside the events)
             ev[i][0].record(stream)
-            h.build(Pd, Jd, Kd)
+            step()
             ev[i][1].record(stream)
-            # per-class launch times of this step (events live in the handle; read before the next build)
+            # per-launch times of this step (events live in the handle; read before the next build)
             ev[i][1].synchronize()
             for cs in h.class_stats():
                 key = (cs["kind"], cs["l"])
                 e = cls_ms.setdefault(key, dict(cs, ms=0.0))
                 e["ms"] += cs["ms"] / args.steps
+            gemm_ms += h.stats()["ms_lr_gemm"] / args.steps
         barrier()
     step_ms = [a.elapsed_time(b) for a, b in ev]
     st = h.stats()
     t = torch.tensor([sum(step_ms)], dtype=torch.float64, device="cuda")
+    q = torch.tensor([st["quartets_j"] + st["quartets_k"]], dtype=torch.float64, device="cuda")
     if world > 1:
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dist.all_reduce(q, op=dist.ReduceOp.SUM)       # every quartet is evaluated by exactly one rank
     total_ms = float(t.item())
     ms_per_step = total_ms / args.steps
-    quartets = st["quartets_j"] + st["quartets_k"]
-    value = world * quartets / (ms_per_step * 1e-3)    # replicas: every rank builds the full J and K
+    quartets = float(q.item())
+    value = quartets / (ms_per_step * 1e-3)
 
     # ---------------- end-to-end leg: host buffers through pbc_jk_build_host ----------------
     h.set_profile(False)
+
+    def step_host():
+        h.build_host_ptr(Ph.data_ptr(), Jh.data_ptr(), Kh.data_ptr())     # synchronous: P up, J and K down
+        if world > 1:                                  # NCCL reduces device memory: partial J, K up again, sums back down
+            Jd.copy_(Jh, non_blocking=True); Kd.copy_(Kh, non_blocking=True)
+            allreduce_jk(Jd, Kd)
+            Jh.copy_(Jd, non_blocking=True); Kh.copy_(Kd, non_blocking=True)
+            torch.cuda.synchronize()
+
     for _ in range(2):
-        h.build_host_ptr(Ph.data_ptr(), Jh.data_ptr(), Kh.data_ptr())
+        step_host()
     barrier()
     t0 = time.perf_counter()
     for _ in range(args.steps):
         flush.zero_()
-        h.build_host_ptr(Ph.data_ptr(), Jh.data_ptr(), Kh.data_ptr())     # synchronous
+        step_host()
     torch.cuda.synchronize()
     e2e_s = (time.perf_counter() - t0) / args.steps
     t = torch.tensor([e2e_s], dtype=torch.float64, device="cuda")
     if world > 1:
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
     e2e_s = float(t.item())
-    dJ = float((Jh.cuda() - Jd).abs().max().item())
-    dK = float((Kh.cuda() - Kd).abs().max().item())
-    assert dJ == 0.0 and dK == 0.0, "host-buffer and device-buffer builds differ"
+    if world == 1:
+        dJ = float((Jh.cuda() - Jd).abs().max().item())
+        dK = float((Kh.cuda() - Kd).abs().max().item())
+        assert dJ == 0.0 and dK == 0.0, "host-buffer and device-buffer builds differ"
 
     if rank == 0:
         peaks, peaks_kind = _peaks()
-        # ---------------- roofline of the dominant real-space kernel class ----------------
-        fp64_meas = fp64_peak_tflops(20000)
+        # ---------------- roofline: both kernel families, the one with the larger share of the step on top ----------------
+        pk = bench_peaks(20000)                        # DFMA / FFMA / DMMA micro-benchmarks on this device, TFLOP/s
         sm_max = float(peaks.get("sm_max_mhz", 1965.0))
-        fp64_nominal = 148 * 64 * 2 * sm_max * 1e6 * 1e-12      # 148 SMs x 64 FP64 FMA lanes x 2 flop x clock
+        fp64_nominal = 148 * 64 * 2 * sm_max * 1e6 * 1e-12      # 148 SMs x 64 FP64 FMA lanes x 2 flop x clock (DESIGN.md 7)
+        fp32_nominal = 2.0 * fp64_nominal
+        # FP64 tensor (DMMA) peak derived as the contract asks: measured bf16 peak x nominal ratio 45 / 2250 TFLOP/s
+        dmma_derived = float(peaks.get("bf16_tflops", 1590.0)) * 45.0 / 2250.0
         rows = sorted(cls_ms.values(), key=lambda c: -c["ms"])
         sr_ms = sum(c["ms"] for c in rows)
         sr_flop = sum(class_flops(c) * c["quartets"] for c in rows)
-        top = rows[0]
-        top_flop = class_flops(top) * top["quartets"]
-        top_tf = top_flop / (top["ms"] * 1e-3) * 1e-12 if top["ms"] > 0 else 0.0
         fam = {}
         for c in rows:
             f = fam.setdefault(c["kind"], {"ms": 0.0, "flop": 0.0, "quartets": 0})
             f["ms"] += c["ms"]; f["flop"] += class_flops(c) * c["quartets"]; f["quartets"] += c["quartets"]
-        roofline = {
-            "bound": "alu", "kernel": f"sr_{top['kind'].lower()}_kernel<{','.join(map(str, top['l']))}>",
-            "achieved": top_tf, "peak": fp64_nominal, "unit": "TFLOP/s", "frac": top_tf / fp64_nominal,
-            "peak_kind": f"FP64 FMA: 148 SM x 64 lanes x 2 x {sm_max:.0f} MHz (DESIGN.md); DFMA micro-benchmark on this box: "
-                         f"{fp64_meas:.2f} TFLOP/s",
-            "traffic": _ncu_traffic(f"sr_{top['kind'].lower()}_kernel<{','.join(map(str, top['l']))}>"),
-            "flop_per_quartet": class_flops(top), "quartets_per_launch": top["quartets"], "ms_per_launch": top["ms"],
-            "share_of_step": top["ms"] / ms_per_step,
-            "real_space_all_classes": {"ms": sr_ms, "tflops": sr_flop / (sr_ms * 1e-3) * 1e-12 if sr_ms > 0 else 0.0,
-                                       "frac": (sr_flop / (sr_ms * 1e-3) * 1e-12 / fp64_nominal) if sr_ms > 0 else 0.0},
-            "families": {k: {"ms": v["ms"], "quartets": v["quartets"],
-                             "tflops": v["flop"] / (v["ms"] * 1e-3) * 1e-12 if v["ms"] > 0 else 0.0} for k, v in fam.items()},
-            # reciprocal-space phase (A7-A9): its dense part is two FP64 tensor-core GEMMs per G batch,
-            # Y = L^T A' (2 r N^2 flop per slot) and K += Y^T Y on the lower triangle (r N (N+1) flop per slot)
-            "reciprocal_space": _lr_roofline(st, n, wl.n_occ, fp64_nominal),
-            "top_classes": [{"kind": c["kind"], "l": list(c["l"]), "ms": round(c["ms"], 3), "quartets": c["quartets"],
-                             "tflops": round(class_flops(c) * c["quartets"] / (c["ms"] * 1e-3) * 1e-12, 3) if c["ms"] > 0 else 0.0}
-                            for c in rows[:8]],
-        }
+        sr_tf = sr_flop / (sr_ms * 1e-3) * 1e-12 if sr_ms > 0 else 0.0
+        # reciprocal-space K (A8): per G slot  Y = L^T A' (2 r N^2 flop)  and  K += Y^T Y on the lower triangle (r N (N+1));
+        # slots = Re and Im of every G of this rank's batches, plus the SELF slot; r = rank of the factor of P'
+        r_p = int(st["rank_p"])
+        slots = 2 * ((st["n_g"] + world - 1) // world if world > 1 else st["n_g"]) + (1 if rank == 0 else 0)
+        gemm_flop = (2.0 * r_p * n * n + r_p * n * (n + 1.0)) * slots
+        gemm_tf = gemm_flop / (gemm_ms * 1e-3) * 1e-12 if gemm_ms > 0 else 0.0
+        n_gemm_launch = 2 * ((st["n_g"] + h_nb(st, n) - 1) // h_nb(st, n) + 1)
+        real_space = {"bound": "alu", "kernel": "sr_k_kernel<*> + sr_j_kernel<*> (one launch per class)", "ms": sr_ms,
+                      "achieved": sr_tf, "peak": fp64_nominal, "unit": "TFLOP/s", "frac": sr_tf / fp64_nominal,
+                      "share_of_step": sr_ms / ms_per_step,
+                      "peak_kind": f"FP64 FMA nominal: 148 SM x 64 lanes x 2 x {sm_max:.0f} MHz; DFMA micro-benchmark on this box "
+                                   f"{pk['fp64_fma']:.2f} TFLOP/s (FFMA {pk['fp32_fma']:.2f})",
+                      "families": {k: {"ms": v["ms"], "quartets": v["quartets"],
+                                       "tflops": v["flop"] / (v["ms"] * 1e-3) * 1e-12 if v["ms"] > 0 else 0.0} for k, v in fam.items()},
+                      "top_classes": [{"kind": c["kind"], "l": list(c["l"]), "ms": round(c["ms"], 3), "quartets": c["quartets"],
+                                       "tflops": round(class_flops(c) * c["quartets"] / (c["ms"] * 1e-3) * 1e-12, 3) if c["ms"] > 0 else 0.0}
+                                      for c in rows[:8]]}
+        if args.precision == "mixed":
+            real_space["fp32_quartets_k"] = st["quartets_k_fp32"]
+            real_space["fp32_share_of_k_quartets"] = st["quartets_k_fp32"] / max(1, st["quartets_k"])
+            real_space["fp32_peak"] = fp32_nominal
+        lr_gemm = {"bound": "tensor", "kernel": "dgemm_kernel<0,0> + dgemm_kernel<0,1> (mma.sync.m8n8k4.f64, one pair per G batch)",
+                   "ms": gemm_ms, "achieved": gemm_tf, "peak": pk["fp64_dmma"], "unit": "TFLOP/s",
+                   "frac": gemm_tf / pk["fp64_dmma"] if pk["fp64_dmma"] > 0 else 0.0, "share_of_step": gemm_ms / ms_per_step,
+                   "peak_kind": f"FP64 tensor (DMMA) micro-benchmark on this box; derived from MEASURED_PEAKS bf16 x 45/2250: "
+                                f"{dmma_derived:.1f} TFLOP/s ({peaks_kind})",
+                   "flop_per_launch_pair": gemm_flop / max(1, n_gemm_launch // 2), "rank_of_P": r_p, "g_slots": slots,
+                   "ms_per_launch_pair": gemm_ms / max(1, n_gemm_launch // 2),
+                   "traffic": _ncu_traffic("dgemm_kernel<0,0>"),
+                   "ms_lr_phase": st["ms_lr"]}
+        top, other = (lr_gemm, real_space) if gemm_ms >= sr_ms else (real_space, lr_gemm)
+        roofline = dict(top)
+        roofline.setdefault("traffic", None)               # not measured for the real-space family (compute-bound: DESIGN.md 7)
+        roofline["other_family"] = other
         # ---------------- CPU baseline: the oracle on a bounded sample ----------------
         cpu = None
         if not args.no_cpu_baseline:
@@ -382,19 +456,22 @@ def main():
             cpu = {"value": q / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
                    "sample": f"real-space part of {nblk} seeded output shell blocks of {args.workload}: {q} primitive quartet-images in {dt:.1f} s "
                              f"(the oracle screens at 1e-18, so it evaluates more quartets per block than the GPU path)"}
+            cpu.update(_extrapolate_oracle(wl, P, nblk, st["n_g"]))
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-            "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak" if world == 1 else "strong",
+            "vs_baseline": None,
             "dtype": "f64" if args.precision == "fp64" else "f64+f32", "data": "synthetic",
             "config": {"workload": args.workload, "natom": wl.natom, "nshell": wl.nshell, "nbf": n, "omega": wl.omega,
                        "n_g_half": st["n_g"], "prim_pair_images": st["n_prim_pairs"], "precision": args.precision,
-                       "l2": "512 MB flush write between timed iterations", "parallelism": "replicas only" if world > 1 else "1 gpu"},
+                       "l2": "512 MB flush write between timed iterations", "parallelism": "1 gpu" if world == 1 else f"one build sharded over {world} GPUs (K blocks, J bras, G batches round-robin) + "
+                                                                           "one all-reduce of [J; K]"},
             "jk_build_seconds": ms_per_step * 1e-3, "create_seconds": st["create_seconds"],
             "quartets_per_step": {"J": st["quartets_j"], "K": st["quartets_k"],
                                   "candidates_J": st["candidates_j"], "candidates_K": st["candidates_k"]},
             "phase_ms": {k: st[k] for k in ("ms_density", "ms_sr_j", "ms_sr_k", "ms_lr", "ms_total")},
             "step_ms": [round(x, 3) for x in step_ms],
-            "e2e": {"value": world * quartets / e2e_s, "unit": UNIT, "ms_per_step": e2e_s * 1e3,
+            "e2e": {"value": quartets / e2e_s, "unit": UNIT, "ms_per_step": e2e_s * 1e3,
                     "h2d_bytes_per_step": n * n * 8, "d2h_bytes_per_step": 2 * n * n * 8},
             "gpu_launches": int(st["n_launches"]) * args.steps,
             "clocks": clocks.summary(), "peaks": peaks_kind,

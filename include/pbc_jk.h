@@ -41,8 +41,9 @@ typedef enum {
     PBC_JK_ERR_INVALID_ARG = -1,   /* null pointer, w <= 0, singular cell, l > 2, exponent <= 0, nprim < 1 */
     PBC_JK_ERR_NOMEM = -2,         /* host or device allocation failed */
     PBC_JK_ERR_CUDA = -3,          /* CUDA runtime error; text via pbc_jk_last_error */
-    PBC_JK_ERR_UNSUPPORTED = -4    /* image index range exceeds the packed format (cell far too small), or      */
-                                   /* precision = 1 (mixed precision is not built yet: fp64 only)                */
+    PBC_JK_ERR_UNSUPPORTED = -4    /* lattice image index range exceeds the packed format (cell far too small for */
+                                   /* the exponents / omega, or max|P| above 1e6), or a (shell, l) group holds    */
+                                   /* more than 65535 primitive pair-images                                       */
 } pbc_jk_status;
 
 typedef struct pbc_jk pbc_jk;      /* opaque handle: owns all host + device state of one geometry */
@@ -70,14 +71,17 @@ typedef struct {
     double d_schwarz;    /* primitive quartet-image evaluated iff bound_bra*bound_ket*max|P|*          */
                          /* exp(-alpha_w r^2) (eq 67) exceeds this; default 1e-13                 */
     double d_ewald_k;    /* sets the default g_cut; default 1e-14                                      */
-    int32_t precision;   /* 0 = fp64 everywhere.  1 = mixed (PAPER 3.5 L817-821: quartets whose       */
-                         /* density-weighted bound is below mixed_switch in fp32, fp64 accumulation)   */
-                         /* is NOT built yet: pbc_jk_create returns PBC_JK_ERR_UNSUPPORTED for it      */
-    double mixed_switch; /* reserved for precision = 1; default 1e-5 (L819)                            */
-    int32_t lr_g_batch;  /* G vectors per reciprocal-space batch (0: sized to <= 12 GB per stack; <=64)*/
+    int32_t precision;   /* 0 = fp64 everywhere.  1 = mixed (PAPER 3.5 L817-821): real-space K quartets */
+                         /* whose density-weighted bound bound_bra*bound_ket*max|P block| is below      */
+                         /* mixed_switch run in fp32 arithmetic with fp64 accumulation; everything else */
+                         /* (J-engine, reciprocal space, quartets above the switch) stays fp64          */
+    double mixed_switch; /* precision = 1 only; default 1e-5 (L819)                                     */
+    int32_t lr_g_batch;  /* G vectors per reciprocal-space batch (0: sized to <= 12 GB per stack; <=64) */
+    double g_min;        /* > 0: only G with |G| >= g_min enter the reciprocal-space sums (selection     */
+                         /* only; tests use it to compare the outermost shell of G at full basis size)   */
 } pbc_cutoffs;
 
-/* Counters and phase times of the LAST pbc_jk_build (times need pbc_jk_sync_stats). */
+/* Counters and phase times of the LAST pbc_jk_build (pbc_jk_get_stats waits for it). */
 typedef struct {
     int32_t nbf, nshell, natom, n_g;        /* n_g: G != 0 in the half sphere (+-G paired, L243)  */
     int64_t n_prim_pairs;                   /* ordered primitive pair-images kept (A2)            */
@@ -87,13 +91,16 @@ typedef struct {
     double  ms_density, ms_sr_j, ms_sr_k, ms_lr, ms_total;   /* device times, CUDA events         */
     double  create_seconds;                 /* host wall time of pbc_jk_create                    */
     int64_t n_launches;                     /* CUDA kernels the last build launched               */
+    int64_t quartets_k_fp32;                /* the part of quartets_k evaluated in fp32 (mixed)   */
+    double  ms_lr_gemm;                     /* profile mode: device time of the K^LR GEMM launches */
+    int32_t rank_p;                         /* rank of the factor P' = L L^T used by K^LR (N: dense fallback) */
 } pbc_jk_stats_t;
 
 /* One real-space kernel class of the LAST build (one launch per class and build).
  * kind 0: J-engine class, l[0] = Hermite order of the bra pair (l_mu + l_nu), l[1] = of the ket pair
  *         (eq 96-98); kind 1: K class (l_mu l_lambda | l_sigma l_nu) in l[0..3] (eq 74).
  * quartets / candidates: primitive quartet-images evaluated / tested (eq 67) by that launch.
- * ms: device time of the launch (CUDA events on the build's stream); 0 unless profile mode is on. */
+ * ms: device time of the launch (CUDA events on the build's stream); 0 unless profile mode was on during that build. */
 typedef struct {
     int32_t kind;
     int32_t l[4];
@@ -136,7 +143,9 @@ int pbc_jk_set_parts(pbc_jk *h, int32_t parts);
 /* waits for the last build on its stream and fills the counters/times */
 int pbc_jk_get_stats(pbc_jk *h, pbc_jk_stats_t *out);
 
-/* profile mode (default off): record a CUDA event pair around every real-space class launch */
+/* profile mode (default off): the real-space class launches run one after the other on the caller's stream with a
+ * CUDA event pair around each (per-class times); otherwise the classes are spread over internal streams that fork
+ * from and join back into the caller's stream, so that the tail of one class overlaps the next */
 int pbc_jk_set_profile(pbc_jk *h, int32_t on);
 
 /* waits for the last build and writes up to `cap` class records to `out` (HOST memory, caller-owned);
@@ -150,9 +159,14 @@ const char *pbc_jk_last_error(const pbc_jk *h);
 /* frees all host and device memory of the handle; NULL is a no-op */
 int pbc_jk_destroy(pbc_jk *h);
 
-/* measurement helper: runs a dependent-free DFMA loop on every SM for `iters` iterations and
- * returns the achieved FP64 TFLOP/s (roofline denominator for the real-space kernels) */
-int pbc_jk_fp64_peak(int32_t iters, double *tflops_out);
+/*
+ * Multi-GPU: this handle does the share `rank` of `nranks` of every build --
+ * real-space K output blocks and J-engine bras dealt round-robin (lists sorted by cost), reciprocal-space
+ * G batches likewise, the SELF term on rank 0 -- so that the SUM over the ranks' J (and K) is the full
+ * matrix: the caller adds them up with one all-reduce (the Python binding does, over torch.distributed).
+ * Default (0, 1): the whole build.
+ */
+int pbc_jk_set_shard(pbc_jk *h, int32_t rank, int32_t nranks);
 
 #ifdef __cplusplus
 }

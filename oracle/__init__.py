@@ -36,7 +36,7 @@ class _System(C.Structure):
 
 class _Opts(C.Structure):
     _fields_ = [("delta_o", C.c_double), ("r_cut", C.c_double), ("g_cut", C.c_double),
-                ("which", C.c_int32), ("parts", C.c_int32)]
+                ("which", C.c_int32), ("parts", C.c_int32), ("g_min", C.c_double)]
 
 
 def _load():
@@ -120,7 +120,7 @@ def overlap(wl, delta_o: float = 1e-18, r_cut: float = 0.0) -> np.ndarray:
 
 def jk(wl, P: np.ndarray, omega: Optional[float] = None, blocks: Optional[Sequence[Tuple[int, int]]] = None,
        delta_o: float = 1e-18, r_cut: Optional[float] = None, g_cut: Optional[float] = None,
-       which: str = "jk", parts: str = "sr+lr+self") -> dict:
+       which: str = "jk", parts: str = "sr+lr+self", g_min: float = 0.0) -> dict:
     """J and K with their SR / LR / SELF parts.
 
     blocks=None: the full matrices.  blocks=[(shell_mu, shell_nu), ...]: only those
@@ -136,6 +136,7 @@ def jk(wl, P: np.ndarray, omega: Optional[float] = None, blocks: Optional[Sequen
     o.delta_o = delta_o
     o.r_cut = float(wl.r_cut if r_cut is None else r_cut)
     o.g_cut = float(wl.g_cut if g_cut is None else g_cut)
+    o.g_min = float(g_min)
     o.which = (1 if "j" in which else 0) | (2 if "k" in which else 0)
     o.parts = (1 if "sr" in parts else 0) | (2 if "lr" in parts else 0) | (4 if "self" in parts else 0)
     om = float(wl.omega if omega is None else omega)

@@ -536,6 +536,8 @@ typedef struct {
     double r_cut;       /* >0: cap on |A-B-T2| and |Q-P+T1| (C-14) */
     double g_cut;       /* >0: |G| cutoff; 0: 2 w sqrt(ln(1/delta_o)) */
     int32_t which, parts;
+    double g_min;       /* >0: only G with |G| >= g_min enter the LR sum (selection only: lets a test compare the */
+                        /* outermost shell of G at full basis size without paying for the whole sphere)           */
 } orc_opts;
 
 static void sr_block(const orc_system *s, const pair_list *pl, const orc_opts *o, double omega,
@@ -663,7 +665,11 @@ int orc_jk(const orc_system *s, double omega, const orc_opts *o, const double *P
             double acell[9]; for (int i = 0; i < 9; ++i) acell[i] = s->cell[i];
             nG = translations_in_sphere(pl.bvec, acell, zero, gcut, &G, NULL);
         }
-        counts[3] = nG - 1;
+        counts[3] = 0;
+        for (int ig = 0; ig < nG; ++ig) {
+            double G2 = G[3 * ig] * G[3 * ig] + G[3 * ig + 1] * G[3 * ig + 1] + G[3 * ig + 2] * G[3 * ig + 2];
+            if (G2 >= 1e-20 && !(o->g_min > 0 && G2 < o->g_min * o->g_min)) counts[3]++;
+        }
         int nthr = 1;
 #ifdef _OPENMP
         nthr = omp_get_max_threads();
@@ -687,6 +693,7 @@ int orc_jk(const orc_system *s, double omega, const orc_opts *o, const double *P
                 const double *Gv = G + 3 * ig;
                 double G2 = Gv[0] * Gv[0] + Gv[1] * Gv[1] + Gv[2] * Gv[2];
                 if (G2 < 1e-20) continue;                                      /* G = 0 omitted (L253) */
+                if (o->g_min > 0 && G2 < o->g_min * o->g_min) continue;        /* window selection (tests)   */
                 double w = 4.0 * M_PI / (pl.vol * G2) * exp(-G2 / (4.0 * omega * omega));
                 memset(Are, 0, 8 * NN); memset(Aim, 0, 8 * NN);
                 double re[36], im[36];

@@ -20,7 +20,8 @@ STATUS = {0: "OK", -1: "INVALID_ARG", -2: "NOMEM", -3: "CUDA", -4: "UNSUPPORTED"
 
 # every symbol include/pbc_jk.h declares (checked by tests/test_abi.py)
 SYMBOLS = ["pbc_jk_create", "pbc_jk_nbf", "pbc_jk_overlap", "pbc_jk_build", "pbc_jk_build_host",
-           "pbc_jk_set_parts", "pbc_jk_get_stats", "pbc_jk_set_profile", "pbc_jk_get_class_stats", "pbc_jk_last_error", "pbc_jk_destroy", "pbc_jk_fp64_peak"]
+           "pbc_jk_set_parts", "pbc_jk_set_shard", "pbc_jk_get_stats", "pbc_jk_set_profile", "pbc_jk_get_class_stats",
+           "pbc_jk_last_error", "pbc_jk_destroy"]
 
 
 class pbc_cell(C.Structure):
@@ -40,7 +41,7 @@ class pbc_shells(C.Structure):
 class pbc_cutoffs(C.Structure):
     _fields_ = [("r_cut", C.c_double), ("g_cut", C.c_double), ("d_pair", C.c_double), ("d_schwarz", C.c_double),
                 ("d_ewald_k", C.c_double), ("precision", C.c_int32), ("mixed_switch", C.c_double),
-                ("lr_g_batch", C.c_int32)]
+                ("lr_g_batch", C.c_int32), ("g_min", C.c_double)]
 
 
 class pbc_jk_stats_t(C.Structure):
@@ -49,7 +50,8 @@ class pbc_jk_stats_t(C.Structure):
                 ("quartets_j", C.c_int64), ("quartets_k", C.c_int64),
                 ("candidates_j", C.c_int64), ("candidates_k", C.c_int64),
                 ("ms_density", C.c_double), ("ms_sr_j", C.c_double), ("ms_sr_k", C.c_double), ("ms_lr", C.c_double),
-                ("ms_total", C.c_double), ("create_seconds", C.c_double), ("n_launches", C.c_int64)]
+                ("ms_total", C.c_double), ("create_seconds", C.c_double), ("n_launches", C.c_int64),
+                ("quartets_k_fp32", C.c_int64), ("ms_lr_gemm", C.c_double), ("rank_p", C.c_int32)]
 
 
 class pbc_jk_class_stat(C.Structure):
@@ -92,8 +94,8 @@ def load() -> C.CDLL:
         lib.pbc_jk_last_error.restype = C.c_char_p
         lib.pbc_jk_destroy.argtypes = [C.c_void_p]
         lib.pbc_jk_destroy.restype = C.c_int
-        lib.pbc_jk_fp64_peak.argtypes = [C.c_int32, C.POINTER(C.c_double)]
-        lib.pbc_jk_fp64_peak.restype = C.c_int
+        lib.pbc_jk_set_shard.argtypes = [C.c_void_p, C.c_int32, C.c_int32]
+        lib.pbc_jk_set_shard.restype = C.c_int
         _lib = lib
     return _lib
 
@@ -115,13 +117,36 @@ def _ip(a):
 _PARTS = {"sr": 1, "lr": 2, "self": 4}
 
 
+def allreduce_jk(J, K, group=None):
+    """The one collective of the sharded build: sum the ranks' partial J and K in place.  One message when J and K
+    sit back to back in memory (allocate them as two halves of one buffer), else one staging copy."""
+    import torch
+    import torch.distributed as dist
+
+    parts = [t for t in (J, K) if t is not None]
+    if not parts or not dist.is_initialized() or dist.get_world_size(group) == 1:
+        return
+    if len(parts) == 2 and J.is_contiguous() and K.is_contiguous() and \
+            J.data_ptr() + J.numel() * J.element_size() == K.data_ptr() and J.untyped_storage().data_ptr() == K.untyped_storage().data_ptr():
+        both = torch.as_strided(J, (J.numel() + K.numel(),), (1,))
+        dist.all_reduce(both, group=group)
+        return
+    buf = torch.cat([t.reshape(-1) for t in parts])
+    dist.all_reduce(buf, group=group)
+    o = 0
+    for t in parts:
+        t.copy_(buf[o:o + t.numel()].view_as(t))
+        o += t.numel()
+
+
 class PbcJK:
     """One geometry: pbc_jk_create ... pbc_jk_destroy.  `wl` is a workloads.Workload (or anything
     with the same fields)."""
 
     def __init__(self, wl, omega: Optional[float] = None, r_cut: Optional[float] = None,
                  g_cut: Optional[float] = None, d_pair: float = 0.0, d_schwarz: Optional[float] = None,
-                 d_ewald_k: float = 0.0, precision: int = 0, mixed_switch: float = 0.0, lr_g_batch: int = 0):
+                 d_ewald_k: float = 0.0, precision: int = 0, mixed_switch: float = 0.0, lr_g_batch: int = 0,
+                 g_min: float = 0.0):
         self._h = C.c_void_p()
         lib = load()
         cell = pbc_cell()
@@ -146,6 +171,7 @@ class PbcJK:
         cut.precision = int(precision)
         cut.mixed_switch = float(mixed_switch)
         cut.lr_g_batch = int(lr_g_batch)
+        cut.g_min = float(g_min)
         om = float(wl.omega if omega is None else omega)
         rc = lib.pbc_jk_create(C.byref(cell), C.byref(atoms), C.byref(shells), om, C.byref(cut), C.byref(self._h))
         if rc != PBC_JK_OK:
@@ -166,6 +192,18 @@ class PbcJK:
         for p in parts.split("+"):
             m |= _PARTS[p.strip()]
         self._check(load().pbc_jk_set_parts(self._h, m))
+
+    def set_shard(self, rank: int = 0, nranks: int = 1):
+        """This handle builds share `rank` of `nranks` of every J and K; the sum over ranks is the full matrix."""
+        self._check(load().pbc_jk_set_shard(self._h, int(rank), int(nranks)))
+        self._shard = (int(rank), int(nranks))
+
+    def build_sharded(self, P, J=None, K=None, group=None):
+        """Multi-GPU build: every rank of `group` holds a handle of the same geometry with
+        set_shard(rank, world) and calls this with the same P; the partial matrices are summed with ONE
+        all-reduce of [J; K] over torch.distributed (NCCL over NVLink on GPUs)."""
+        self.build(P, J, K)
+        allreduce_jk(J, K, group)
 
     def build(self, P, J=None, K=None, stream=None):
         """Device tensors (torch, float64, contiguous N x N).  Enqueues on `stream` (default: torch's
@@ -237,9 +275,22 @@ class PbcJK:
         self.close()
 
 
-def fp64_peak_tflops(iters: int = 20000) -> float:
-    out = C.c_double()
-    rc = load().pbc_jk_fp64_peak(int(iters), C.byref(out))
-    if rc != PBC_JK_OK:
-        raise PbcJKError(rc, "fp64 peak measurement failed")
-    return float(out.value)
+PEAKS_LIB_PATH = os.path.join(_HERE, "libpbc_jk_benchpeaks.so")
+
+
+def bench_peaks(iters: int = 20000) -> dict:
+    """bench.py's roofline denominators measured on the current device (helper library outside the product ABI):
+    FP64 FMA, FP32 FMA and FP64 tensor-core (DMMA) TFLOP/s."""
+    if not os.path.exists(PEAKS_LIB_PATH):
+        raise RuntimeError(f"{PEAKS_LIB_PATH} is missing: build it with `python -m paper_2410_22278_b200.build`")
+    lib = C.CDLL(PEAKS_LIB_PATH)
+    out = {}
+    for name in ("fp64_fma", "fp32_fma", "fp64_dmma"):
+        f = getattr(lib, f"bench_{name}_peak")
+        f.argtypes = [C.c_int32, C.POINTER(C.c_double)]
+        f.restype = C.c_int
+        v = C.c_double()
+        if f(int(iters), C.byref(v)) != 0:
+            raise RuntimeError(f"bench_{name}_peak failed (no CUDA device?)")
+        out[name] = float(v.value)
+    return out

@@ -9,6 +9,7 @@
 #include <chrono>
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <limits>
 #include <new>
@@ -59,6 +60,7 @@ struct pbc_jk {
     std::string err;
     DevPool pool;
     int N = 0, Np = 0, nshell = 0, natom = 0, nG = 0;
+    int device = 0, nsm = 148;           // the CUDA device the handle lives on (current device at create)
     int parts = 7;
     pbc_cutoffs cut{};
     Lattice lat{};
@@ -67,7 +69,7 @@ struct pbc_jk {
     PairListU U{};
     KetListJ KJ{};
     LRParams lr{};
-    const double *boys = nullptr;
+    BoysTab boys{};
     const double *fcomp = nullptr;
     const int *shell_of_ao = nullptr;
     // J bra index lists per Hermite order, K block lists per (la, ld)
@@ -77,6 +79,10 @@ struct pbc_jk {
     int nkblk[3][3] = {};
     // workspaces
     double *Pp = nullptr, *lnPmax = nullptr, *Dt = nullptr, *Jt = nullptr, *Jsr = nullptr, *Jlr = nullptr;
+    float *Ppf = nullptr, *lnPblk = nullptr, *lnProw = nullptr, *kjP = nullptr;   // fp32 P' (mixed), per-block ln max|P'|
+    bool mixed = false;                  // precision = 1: fp32 K quartets below the switch (PAPER 3.5)
+    double mixed_switch = 1e-5;
+    int shard_rank = 0, shard_n = 1;     // multi-GPU share of every build (pbc_jk_set_shard)
     double *Ksr = nullptr, *Klr = nullptr, *Astack = nullptr, *Zstack = nullptr, *rho = nullptr;
     double *hostP = nullptr, *hostJ = nullptr, *hostK = nullptr;     // device staging of build_host
     double *LT = nullptr, *chol_d = nullptr, *chol_s = nullptr;      // factor P' = L L^T of the K^LR contraction
@@ -91,7 +97,12 @@ struct pbc_jk {
     // per-class events of the real-space launches (profile mode): [cls][start, stop]
     cudaEvent_t evJ[NCLS_J][2] = {}, evK[NCLS_K][2] = {};
     bool ranJ[NCLS_J] = {}, ranK[NCLS_K] = {};
+    std::vector<cudaEvent_t> evG;        // profile mode: event pairs around the two K^LR GEMMs of every G batch (+ SELF)
+    int n_evG = 0;                       // pairs recorded by the last build
     bool profile = false;
+    bool profiled_last = false;          // profile mode was on during the last build (the class events are recorded)
+    bool debug_sync = false;             // env PBC_JK_DEBUG_SYNC=1: synchronise after every real-space class launch and name
+                                         // the class in the error text (bring-up aid; breaks the no-host-sync contract)
     int64_t n_launches = 0;
     cudaStream_t last_stream = nullptr;
     bool built = false;
@@ -184,6 +195,8 @@ void destroy_events(pbc_jk *h)
 {
     for (auto &e : h->ev)
         if (e) cudaEventDestroy(e);
+    for (auto &e : h->evG)
+        if (e) cudaEventDestroy(e);
     for (auto &e : h->evJ)
         for (auto &x : e)
             if (x) cudaEventDestroy(x);
@@ -214,6 +227,15 @@ int setup(pbc_jk *h, const pbc_cell *cell, const pbc_atoms *atoms, const pbc_she
     // ---- basis bookkeeping ----
     const int ns = shells->nshell, natom = atoms->natom;
     h->nshell = ns; h->natom = natom;
+    // every centre may be given in any lattice image (L781): fold all of them into the home cell, so that the
+    // lattice indices the real-space scans enumerate stay inside the packed 10-bit range checked below
+    std::vector<double> axyz(3 * (size_t)natom);
+    for (int a = 0; a < natom; ++a) {
+        const double *r = atoms->xyz + 3 * a;
+        double f[3];
+        for (int k = 0; k < 3; ++k) f[k] = std::floor(lat.binv[3 * k] * r[0] + lat.binv[3 * k + 1] * r[1] + lat.binv[3 * k + 2] * r[2]);
+        for (int x = 0; x < 3; ++x) axyz[3 * a + x] = r[x] - (f[0] * lat.a[x] + f[1] * lat.a[3 + x] + f[2] * lat.a[6 + x]);
+    }
     std::vector<int> sh_l(ns), sh_ao(ns), sh_atom(ns);
     std::vector<double> scx(ns), scy(ns), scz(ns);
     int nbf = 0, nprim_tot = 0;
@@ -223,10 +245,11 @@ int setup(pbc_jk *h, const pbc_cell *cell, const pbc_atoms *atoms, const pbc_she
         if (l < 0 || l > LMAX) return fail(h, PBC_JK_ERR_INVALID_ARG, "shell angular momentum outside 0..2");
         if (shells->nprim[s] < 1) return fail(h, PBC_JK_ERR_INVALID_ARG, "shell without primitives");
         if (shells->atom[s] < 0 || shells->atom[s] >= natom) return fail(h, PBC_JK_ERR_INVALID_ARG, "shell atom index out of range");
+        if (shells->prim_off[s] < 0) return fail(h, PBC_JK_ERR_INVALID_ARG, "negative prim_off");
         sh_l[s] = l; sh_ao[s] = nbf; sh_atom[s] = shells->atom[s];
         h->has_l[l] = true;
         nbf += ncart(l);
-        scx[s] = atoms->xyz[3 * sh_atom[s]]; scy[s] = atoms->xyz[3 * sh_atom[s] + 1]; scz[s] = atoms->xyz[3 * sh_atom[s] + 2];
+        scx[s] = axyz[3 * sh_atom[s]]; scy[s] = axyz[3 * sh_atom[s] + 1]; scz[s] = axyz[3 * sh_atom[s] + 2];
         for (int k = 0; k < shells->nprim[s]; ++k) {
             const double a = shells->exps[shells->prim_off[s] + k];
             if (!(a > 0.0)) return fail(h, PBC_JK_ERR_INVALID_ARG, "non-positive exponent");
@@ -255,9 +278,11 @@ int setup(pbc_jk *h, const pbc_cell *cell, const pbc_atoms *atoms, const pbc_she
     const double fmaxl[3] = {1.0, 1.0, std::sqrt(3.0)};
     std::vector<std::vector<HostPair>> per_shell(ns);
     std::vector<int64_t> sp_images(ns, 0);
-    bool bad_range = false;
+    bool omp_failed = false;             // no exception may leave an OpenMP region: caught inside, reported after
+    bool range_failed = false;
 #pragma omp parallel for schedule(dynamic, 4)
     for (int A = 0; A < ns; ++A) {
+      try {
         std::vector<HostPair> &out = per_shell[A];
         const double RA[3] = {scx[A], scy[A], scz[A]};
         const int la = sh_l[A];
@@ -303,6 +328,15 @@ int setup(pbc_jk *h, const pbc_cell *cell, const pbc_atoms *atoms, const pbc_she
                     pp.push_back(q);
                 }
             if (rmax <= 0.0) continue;
+            // a cell far too small for this pair's reach would enumerate millions of images (and later overflow the packed
+            // lattice indices of the scans): refuse before enumerating
+            const double rr = rmax + std::sqrt(d0[0] * d0[0] + d0[1] * d0[1] + d0[2] * d0[2]);
+            if (rr * std::max(lat.bnorm[0], std::max(lat.bnorm[1], lat.bnorm[2])) > 400.0 ||
+                (2.0 * rmax * lat.bnorm[0] + 1.0) * (2.0 * rmax * lat.bnorm[1] + 1.0) * (2.0 * rmax * lat.bnorm[2] + 1.0) > 2.0e6) {
+#pragma omp atomic write
+                range_failed = true;
+                continue;
+            }
             for_images_host(lat, d0, rmax, [&](const double *T) {
                 const double Bt[3] = {RBm[0] + T[0], RBm[1] + T[1], RBm[2] + T[2]};
                 const double AB[3] = {RA[0] - Bt[0], RA[1] - Bt[1], RA[2] - Bt[2]};
@@ -330,8 +364,15 @@ int setup(pbc_jk *h, const pbc_cell *cell, const pbc_atoms *atoms, const pbc_she
                 if (any) ++sp_images[A];
             });
         }
+      } catch (...) {
+#pragma omp atomic write
+        omp_failed = true;
+      }
     }
-    (void)bad_range;
+    if (omp_failed) return fail(h, PBC_JK_ERR_NOMEM, "host allocation failed while building the pair list");
+    if (range_failed)
+        return fail(h, PBC_JK_ERR_UNSUPPORTED, "lattice image range of the pair list exceeds the packed format "
+                                               "(cell far too small for these exponents)");
     (void)amin_all;
     // K order: (A, l_B, bound descending)
     std::vector<HostPair> kp;
@@ -380,10 +421,19 @@ int setup(pbc_jk *h, const pbc_cell *cell, const pbc_atoms *atoms, const pbc_she
         CK(pool.upload(&K.coef, soa(kp, 3, 0))); CK(pool.upload(&K.lb, soa(kp, 4, 0)));
         CK(pool.upload(&K.PAx, soa(kp, 5, 0))); CK(pool.upload(&K.PAy, soa(kp, 5, 1))); CK(pool.upload(&K.PAz, soa(kp, 5, 2)));
         CK(pool.upload(&K.PBx, soa(kp, 6, 0))); CK(pool.upload(&K.PBy, soa(kp, 6, 1))); CK(pool.upload(&K.PBz, soa(kp, 6, 2)));
-        std::vector<int> aoB(kp.size()), off(ns * 3 + 1, 0);
+        std::vector<int> aoB(kp.size()), shB(kp.size()), off(ns * 3 + 1, 0);
         std::vector<double> ext(ns * 3, 0.0), ipmax(ns * 3, 0.0);
+        std::vector<float4> q4(kp.size());
+        std::vector<float> ipf(kp.size()), rng(kp.size());
         for (size_t i = 0; i < kp.size(); ++i) {
             aoB[i] = sh_ao[kp[i].shB];
+            shB[i] = kp[i].shB;
+            // fp32 screen record, rounded so that it never undercuts the fp64 values (bound and 1/p rounded up)
+            q4[i] = make_float4((float)kp[i].PA[0], (float)kp[i].PA[1], (float)kp[i].PA[2],
+                                std::nextafter((float)kp[i].lb, std::numeric_limits<float>::infinity()));
+            ipf[i] = std::nextafter((float)kp[i].ip, std::numeric_limits<float>::infinity());
+            rng[i] = (float)(std::log(std::max(std::fabs(kp[i].coef), 1e-300)) +
+                             (sh_l[kp[i].shA] + sh_l[kp[i].shB]) * std::log(2.0 * kp[i].p));
             const int g = kp[i].shA * 3 + sh_l[kp[i].shB];
             off[g + 1]++;
             const double e = std::sqrt(kp[i].PA[0] * kp[i].PA[0] + kp[i].PA[1] * kp[i].PA[1] + kp[i].PA[2] * kp[i].PA[2]);
@@ -391,6 +441,33 @@ int setup(pbc_jk *h, const pbc_cell *cell, const pbc_atoms *atoms, const pbc_she
             ipmax[g] = std::max(ipmax[g], kp[i].ip);
         }
         for (int g = 0; g < ns * 3; ++g) off[g + 1] += off[g];
+        for (int g = 0; g < ns * 3; ++g)
+            if (off[g + 1] - off[g] > 65535)
+                return fail(h, PBC_JK_ERR_UNSUPPORTED, "a (shell, l) group holds more than 65535 primitive pair-images "
+                                                       "(the survivor rings pack bra and ket indices into 16 bits each)");
+        // The scans pack a lattice index into 10 bits per direction (pack_img, |n| <= 511).  Largest index they can
+        // reach: (reach of the screen for the strongest bra and ket at max|P'| = e^{LN_PMAX_CAP}, plus the largest
+        // offset between a bra centre and a ket group centre) * |b_k|/2pi.  A density above the cap is caught on
+        // the device (lnpmax_kernel sets the overflow flag; the build then reports PBC_JK_ERR_UNSUPPORTED).
+        {
+            double lbmax = -1e300, ipm = 0.0, extm = 0.0;
+            for (size_t i = 0; i < kp.size(); ++i) lbmax = std::max(lbmax, kp[i].lb);
+            for (int g = 0; g < ns * 3; ++g) { ipm = std::max(ipm, ipmax[g]); extm = std::max(extm, ext[g]); }
+            const double ln_tau = std::log(cut.d_schwarz > 0 ? cut.d_schwarz : 1e-13);
+            const double budget = std::max(0.0, 2.0 * lbmax + LN_PMAX_CAP - ln_tau);
+            const double reach = std::sqrt(budget * (2.0 * ipm + lat.iomega2)) + extm;
+            double diag = 0.0;
+            for (int sx = -1; sx <= 1; sx += 2)
+                for (int sy = -1; sy <= 1; sy += 2) {
+                    double v[3];
+                    for (int x = 0; x < 3; ++x) v[x] = lat.a[x] + sx * lat.a[3 + x] + sy * lat.a[6 + x];
+                    diag = std::max(diag, std::sqrt(v[0] * v[0] + v[1] * v[1] + v[2] * v[2]));
+                }
+            const double bn = std::max(lat.bnorm[0], std::max(lat.bnorm[1], lat.bnorm[2]));
+            if (!kp.empty() && (reach + diag + 2.0 * extm) * bn + 2.0 > 511.0)
+                return fail(h, PBC_JK_ERR_UNSUPPORTED, "lattice image range of the real-space sums exceeds the packed format "
+                                                       "(cell far too small for these exponents / omega)");
+        }
         // E-product table rows (eq 16-20), filled on the device (etab_kernel)
         {
             auto eterms = [](int l1, int l2) {
@@ -414,9 +491,17 @@ int setup(pbc_jk *h, const pbc_cell *cell, const pbc_atoms *atoms, const pbc_she
             CK(pool.upload(&dlA, lA)); CK(pool.upload(&dlB, lB));
             K.etab = etab;
             launch_etab(K, dlA, dlB, etab, 0);
+            K.etabf = nullptr;
+            if (h->mixed) {                       // fp32 copy for the float evaluators (PAPER 3.5)
+                float *etabf = nullptr;
+                CK(pool.alloc(&etabf, (size_t)tot));
+                launch_to_float(etab, etabf, (size_t)tot, 0);
+                K.etabf = etabf;
+            }
             CK(cudaGetLastError());
         }
-        CK(pool.upload(&K.aoB, aoB)); CK(pool.upload(&K.off, off));
+        CK(pool.upload(&K.aoB, aoB)); CK(pool.upload(&K.shB, shB)); CK(pool.upload(&K.off, off));
+        CK(pool.upload(&K.q4, q4)); CK(pool.upload(&K.ipf, ipf)); CK(pool.upload(&K.rng, rng));
         CK(pool.upload(&K.ext, ext)); CK(pool.upload(&K.ipmax, ipmax));
         // K block lists per (la >= ld), heaviest first
         std::vector<int64_t> cnt(ns, 0);
@@ -503,12 +588,18 @@ int setup(pbc_jk *h, const pbc_cell *cell, const pbc_atoms *atoms, const pbc_she
         });
         const size_t n = idx.size();
         std::vector<double> Qx(n), Qy(n), Qz(n), q(n), iq(n), coef(n), lb(n);
-        std::vector<int> off(natom * 5 + 1, 0);
+        std::vector<int> off(natom * 5 + 1, 0), spA(n), spB(n);
+        std::vector<float4> jq4(n);
+        std::vector<float> iqf(n);
         std::vector<double> ext(natom * 5, 0.0), iqmax(natom * 5, 0.0), gx(natom), gy(natom), gz(natom);
-        for (int a = 0; a < natom; ++a) { gx[a] = atoms->xyz[3 * a]; gy[a] = atoms->xyz[3 * a + 1]; gz[a] = atoms->xyz[3 * a + 2]; }
+        for (int a = 0; a < natom; ++a) { gx[a] = axyz[3 * a]; gy[a] = axyz[3 * a + 1]; gz[a] = axyz[3 * a + 2]; }
         for (size_t j = 0; j < n; ++j) {
             const HostPair &e = up[idx[j]];
             Qx[j] = e.P[0]; Qy[j] = e.P[1]; Qz[j] = e.P[2]; q[j] = e.p; iq[j] = e.ip; coef[j] = e.coef; lb[j] = klb(idx[j]);
+            spA[j] = e.shA; spB[j] = e.shB;
+            jq4[j] = make_float4((float)e.PA[0], (float)e.PA[1], (float)e.PA[2],        // Q - atom of the home shell
+                                 std::nextafter((float)lb[j], std::numeric_limits<float>::infinity()));
+            iqf[j] = std::nextafter((float)e.ip, std::numeric_limits<float>::infinity());
             const int g = sh_atom[e.shA] * 5 + sh_l[e.shA] + sh_l[e.shB];
             off[g + 1]++;
             ext[g] = std::max(ext[g], std::sqrt(e.PA[0] * e.PA[0] + e.PA[1] * e.PA[1] + e.PA[2] * e.PA[2]));
@@ -522,6 +613,32 @@ int setup(pbc_jk *h, const pbc_cell *cell, const pbc_atoms *atoms, const pbc_she
         CK(pool.upload(&KJ.uidx, idx)); CK(pool.upload(&KJ.off, off));
         CK(pool.upload(&KJ.ext, ext)); CK(pool.upload(&KJ.iqmax, iqmax));
         CK(pool.upload(&KJ.gx, gx)); CK(pool.upload(&KJ.gy, gy)); CK(pool.upload(&KJ.gz, gz));
+        CK(pool.upload(&KJ.q4, jq4)); CK(pool.upload(&KJ.iqf, iqf)); CK(pool.upload(&KJ.spA, spA)); CK(pool.upload(&KJ.spB, spB));
+        // group records of the level-A screen; reference point g0 = cell centre (the atoms were folded into the cell)
+        std::vector<int2> goff(natom * 5);
+        std::vector<float4> grec(natom * 5), g4(natom);
+        for (int x = 0; x < 3; ++x) KJ.g0[x] = 0.5 * (lat.a[x] + lat.a[3 + x] + lat.a[6 + x]);
+        KJ.rc = 0.0;
+        for (int a = 0; a < natom; ++a) {
+            const double d[3] = {gx[a] - KJ.g0[0], gy[a] - KJ.g0[1], gz[a] - KJ.g0[2]};
+            KJ.rc = std::max(KJ.rc, std::sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]));
+            g4[a] = make_float4((float)d[0], (float)d[1], (float)d[2], 0.f);
+        }
+        for (int k = 0; k < 5; ++k) { KJ.lbmax[k] = -1e30f; KJ.iqmaxall[k] = 0.f; KJ.extmax[k] = 0.f; }
+        for (int g = 0; g < natom * 5; ++g) {
+            const int cnt = off[g + 1] - off[g], k = g % 5;
+            goff[g] = make_int2(off[g], cnt);
+            const float lbm = cnt > 0 ? jq4[off[g]].w : -1e30f;
+            const float exf = std::nextafter((float)ext[g], std::numeric_limits<float>::infinity());
+            const float iqm = std::nextafter((float)iqmax[g], std::numeric_limits<float>::infinity());
+            grec[g] = make_float4(exf, iqm, lbm, 0.f);
+            if (cnt > 0) {
+                KJ.lbmax[k] = std::max(KJ.lbmax[k], lbm);
+                KJ.iqmaxall[k] = std::max(KJ.iqmaxall[k], iqm);
+                KJ.extmax[k] = std::max(KJ.extmax[k], exf);
+            }
+        }
+        CK(pool.upload(&KJ.goff, goff)); CK(pool.upload(&KJ.grec, grec)); CK(pool.upload(&KJ.g4, g4));
     }
     // ---- shells, component factors ----
     {
@@ -550,6 +667,7 @@ int setup(pbc_jk *h, const pbc_cell *cell, const pbc_atoms *atoms, const pbc_she
                         G[x] = 2.0 * M_PI * (m0 * lat.binv[x] + m1 * lat.binv[3 + x] + m2 * lat.binv[6 + x]);
                     const double G2 = G[0] * G[0] + G[1] * G[1] + G[2] * G[2];
                     if (G2 >= gcut * gcut) continue;
+                    if (cut.g_min > 0 && G2 < cut.g_min * cut.g_min) continue;           // window selection (tests)
                     Gx.push_back(G[0]); Gy.push_back(G[1]); Gz.push_back(G[2]);
                     Gw.push_back(std::sqrt(2.0 * 4.0 * M_PI / (lat.volume * G2) * std::exp(-G2 / (4.0 * omega * omega))));
                 }
@@ -558,11 +676,24 @@ int setup(pbc_jk *h, const pbc_cell *cell, const pbc_atoms *atoms, const pbc_she
         CK(pool.upload(&lr.Gx, Gx)); CK(pool.upload(&lr.Gy, Gy)); CK(pool.upload(&lr.Gz, Gz)); CK(pool.upload(&lr.Gw, Gw));
         lr.U = h->U; lr.sh = h->sh; lr.lat = lat; lr.N = nbf; lr.Np = h->Np; lr.fcomp = h->fcomp;
     }
-    // ---- Boys table ----
+    // ---- Boys tables: Taylor coefficients c[L][i][k] = F_{L+k}(x_i)/k! per top order L, and exp(-x_i) ----
     {
-        std::vector<double> tab((size_t)BOYS_ROWS * BOYS_MCOL);
-        for (int i = 0; i < BOYS_ROWS; ++i) boys_host(BOYS_MCOL - 1, i * BOYS_DX, &tab[(size_t)i * BOYS_MCOL]);
-        CK(pool.upload(&h->boys, tab));
+        std::vector<double> c((size_t)(LTOT + 1) * BOYS_ROWS * 8), ex(BOYS_ROWS);
+        std::vector<float> cf(c.size());
+        double F[BOYS_MCOL];
+        const double ifact[8] = {1.0, 1.0, 0.5, 1.0 / 6, 1.0 / 24, 1.0 / 120, 1.0 / 720, 1.0 / 5040};
+        for (int i = 0; i < BOYS_ROWS; ++i) {
+            boys_host(BOYS_MCOL - 1, i * BOYS_DX, F);
+            ex[i] = std::exp(-i * BOYS_DX);
+            for (int L = 0; L <= LTOT; ++L)
+                for (int k = 0; k < 8; ++k) {
+                    const size_t at = ((size_t)L * BOYS_ROWS + i) * 8 + k;
+                    c[at] = F[L + k] * ifact[k];
+                    cf[at] = (float)c[at];
+                }
+        }
+        static_assert(LTOT + 7 < BOYS_MCOL, "the Taylor rows need F up to order LTOT + 7");
+        CK(pool.upload(&h->boys.c, c)); CK(pool.upload(&h->boys.ex, ex)); CK(pool.upload(&h->boys.cf, cf));
     }
     // ---- workspaces ----
     {
@@ -576,8 +707,7 @@ int setup(pbc_jk *h, const pbc_cell *cell, const pbc_atoms *atoms, const pbc_she
         // split of the K^LR accumulation over the rows of the factor: the lower 128x128 tiles times nsplit should
         // fill whole waves of one CTA per SM
         {
-            int nsm = 148;
-            cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, 0);
+            const int nsm = h->nsm;
             const long tiles = (long)(Np / 128) * (Np / 128 + 1) / 2;
             double best = 0.0;
             h->nsplit = 1;
@@ -589,6 +719,9 @@ int setup(pbc_jk *h, const pbc_cell *cell, const pbc_atoms *atoms, const pbc_she
         }
         CK(pool.alloc(&h->Pp, Np * Np)); CK(cudaMemset(h->Pp, 0, Np * Np * 8));
         CK(pool.alloc(&h->lnPmax, 1)); CK(pool.alloc(&h->maxbits, 1));
+        CK(pool.alloc(&h->lnPblk, (size_t)ns * ns)); CK(pool.alloc(&h->lnProw, (size_t)ns));
+        CK(pool.alloc(&h->kjP, (size_t)std::max(h->KJ.n, 1)));
+        if (h->mixed) { CK(pool.alloc(&h->Ppf, Np * Np)); CK(cudaMemset(h->Ppf, 0, Np * Np * sizeof(float))); }
         CK(pool.alloc(&h->counters, CNT_N)); CK(cudaMemset(h->counters, 0, CNT_N * 8));
         CK(pool.alloc(&h->Dt, (size_t)nherm(4) * h->KJ.dstride));
         CK(pool.alloc(&h->Jt, (size_t)nherm(4) * std::max(h->U.n, 1)));
@@ -601,6 +734,12 @@ int setup(pbc_jk *h, const pbc_cell *cell, const pbc_atoms *atoms, const pbc_she
         CK(pool.alloc(&h->chol_dyn, 4));
         CK(pool.alloc(&h->hostP, N * N)); CK(pool.alloc(&h->hostJ, N * N)); CK(pool.alloc(&h->hostK, N * N));
         for (auto &e : h->ev) CK(cudaEventCreate(&e));
+        h->evG.assign(2 * ((size_t)(h->nG + h->nb - 1) / h->nb + 2), nullptr);
+        for (auto &e : h->evG) CK(cudaEventCreate(&e));
+        // dynamic shared memory opt-in of the big kernels: per device, so once per handle
+        sr_k_set_attributes();
+        dgemm_set_attributes();
+        CK(cudaGetLastError());
         for (auto &e : h->evJ) { CK(cudaEventCreate(&e[0])); CK(cudaEventCreate(&e[1])); }
         for (auto &e : h->evK) { CK(cudaEventCreate(&e[0])); CK(cudaEventCreate(&e[1])); }
     }
@@ -635,11 +774,23 @@ int pbc_jk_create(const pbc_cell *cell, const pbc_atoms *atoms, const pbc_shells
         cudaGetLastError();
         return fail(nullptr, PBC_JK_ERR_CUDA, "no CUDA device: libpbc_jk has no CPU fallback");
     }
-    if (cut && cut->precision != 0)
-        return fail(nullptr, PBC_JK_ERR_UNSUPPORTED, "precision = 1 (mixed fp32/fp64 quartets) is not implemented: fp64 only");
+    if (cut && (cut->precision < 0 || cut->precision > 1))
+        return fail(nullptr, PBC_JK_ERR_INVALID_ARG, "precision must be 0 (fp64) or 1 (mixed)");
     pbc_jk *h = new (std::nothrow) pbc_jk();
     if (!h) return fail(nullptr, PBC_JK_ERR_NOMEM, "host allocation failed");
     if (cut) h->cut = *cut;
+    h->mixed = h->cut.precision == 1;
+    {
+        const char *dbg = std::getenv("PBC_JK_DEBUG_SYNC");
+        h->debug_sync = dbg && dbg[0] == '1';
+    }
+    h->mixed_switch = h->cut.mixed_switch > 0 ? h->cut.mixed_switch : 1e-5;
+    if (cudaGetDevice(&h->device) != cudaSuccess ||
+        cudaDeviceGetAttribute(&h->nsm, cudaDevAttrMultiProcessorCount, h->device) != cudaSuccess) {
+        cudaGetLastError();
+        delete h;
+        return fail(nullptr, PBC_JK_ERR_CUDA, "cannot query the current CUDA device");
+    }
     const auto t0 = std::chrono::steady_clock::now();
     int rc;
     try {
@@ -677,74 +828,113 @@ int pbc_jk_set_parts(pbc_jk *h, int32_t parts)
     return PBC_JK_OK;
 }
 
+int pbc_jk_set_shard(pbc_jk *h, int32_t rank, int32_t nranks)
+{
+    if (!h || nranks < 1 || rank < 0 || rank >= nranks) return PBC_JK_ERR_INVALID_ARG;
+    h->shard_rank = rank;
+    h->shard_n = nranks;
+    return PBC_JK_OK;
+}
+
 int pbc_jk_build(pbc_jk *h, const double *P, double *J, double *K, void *cuda_stream)
 {
     if (!h) return PBC_JK_ERR_INVALID_ARG;
     if (!P) return fail(h, PBC_JK_ERR_INVALID_ARG, "P is null");
+    {
+        int dev = -1;
+        CK(cudaGetDevice(&dev));
+        if (dev != h->device) return fail(h, PBC_JK_ERR_INVALID_ARG, "the handle was created on another CUDA device than the current one");
+    }
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const int N = h->N, Np = h->Np;
     const size_t NN = (size_t)N * N;
-    const bool doSR = h->parts & 1, doLR = h->parts & 2, doSELF = h->parts & 4;
+    const bool doSR = h->parts & 1, doLR = h->parts & 2, doSELF = (h->parts & 4) && h->shard_rank == 0;
+    const bool prof = h->profile;
     CK(cudaMemsetAsync(h->counters, 0, CNT_N * 8, st));
     CK(cudaEventRecord(h->ev[0], st));
     int64_t nl = 0;                      // kernels launched by this build
     for (auto &b : h->ranJ) b = false;
     for (auto &b : h->ranK) b = false;
-    nl += 2;
-    launch_scale_density(P, h->Pp, N, Np, h->fcomp, h->maxbits, h->lnPmax, st);
+    // ---- A4: density prep ----
+    launch_scale_density(P, h->Pp, h->mixed ? h->Ppf : nullptr, N, Np, h->fcomp, h->maxbits, h->lnPmax, h->counters + CNT_FLAG, st);
+    launch_density_blocks(h->Pp, Np, h->sh, h->KJ, h->lnPblk, h->lnProw, h->kjP, st);
+    nl += 4 + (h->KJ.n > 0);
     SRParams sp;
     sp.K = h->K; sp.U = h->U; sp.KJ = h->KJ; sp.lat = h->lat; sp.sh = h->sh;
-    sp.boys = h->boys; sp.Pp = h->Pp; sp.ldP = Np; sp.Dt = h->Dt; sp.Jt = h->Jt; sp.Ksr = h->Ksr;
-    sp.lnPmax = h->lnPmax;
+    sp.boys = h->boys; sp.Pp = h->Pp; sp.Ppf = h->Ppf; sp.ldP = Np; sp.Dt = h->Dt; sp.Jt = h->Jt; sp.Ksr = h->Ksr;
+    sp.lnPmax = h->lnPmax; sp.lnPblk = h->lnPblk; sp.lnProw = h->lnProw; sp.kjP = h->kjP;
     sp.ln_tau = std::log(h->cut.d_schwarz > 0 ? h->cut.d_schwarz : 1e-13);
     sp.rcut2 = h->cut.r_cut > 0 ? h->cut.r_cut * h->cut.r_cut : std::numeric_limits<double>::infinity();
+    sp.ln_switch = (float)std::log(h->mixed_switch);
+    sp.shard_rank = h->shard_rank; sp.shard_n = h->shard_n;
     sp.counters = h->counters;
     if (J && doSR && h->KJ.n > 0) {
         launch_hermite_density(h->U, h->sh, h->KJ, h->Pp, Np, h->Dt, st);
         ++nl;
     }
-    CK(cudaEventRecord(h->ev[1], st));
-    // ---- A5: real-space J ----
     if (J && doSR) {
         CK(cudaMemsetAsync(h->Jt, 0, (size_t)nherm(4) * std::max(h->U.n, 1) * 8, st));
         CK(cudaMemsetAsync(h->Jsr, 0, NN * 8, st));
-        for (int LB = 0; LB <= 4; ++LB)
-            for (int LK = 0; LK <= 4; ++LK) {
-                if (h->njbra[LB] <= 0 || h->njbra[LK] <= 0) continue;
-                const int cls = LB * 5 + LK;
-                if (h->profile) CK(cudaEventRecord(h->evJ[cls][0], st));
-                launch_sr_j(LB, LK, sp, h->jbra[LB], h->njbra[LB], st);
-                if (h->profile) CK(cudaEventRecord(h->evJ[cls][1], st));
-                h->ranJ[cls] = true;
-                ++nl;
-            }
-        if (h->U.nsp > 0) {
-            launch_j_backtransform(h->U, h->sh, h->Jt, h->Jsr, N, st);
-            ++nl;
-        }
     }
-    CK(cudaEventRecord(h->ev[2], st));
-    // ---- A6: real-space K ----
+    if (K && doSR) CK(cudaMemsetAsync(h->Ksr, 0, NN * 8, st));
+    CK(cudaEventRecord(h->ev[1], st));
+    // ---- A5 / A6: real-space classes, one launch each on the caller's stream, heaviest first (profile mode adds an event
+    // pair per launch).  Spreading the classes over internal streams was measured SLOWER on B200 (water64 real space:
+    // 573 ms on one stream, 685 / 724 ms on 2 / 3 streams -- kernels of different classes sharing an SM evict each
+    // other's evaluator code from the instruction cache), so there is no fork/join here.
     if (K && doSR) {
-        CK(cudaMemsetAsync(h->Ksr, 0, NN * 8, st));
-        for (int la = LMAX; la >= 0; --la)
-            for (int ld = la; ld >= 0; --ld)
-                for (int lb = LMAX; lb >= 0; --lb)
-                    for (int lc = LMAX; lc >= 0; --lc) {
+        for (int L = 4 * LMAX; L >= 0; --L)                       // heaviest classes first
+            for (int la = LMAX; la >= 0; --la)
+                for (int ld = la; ld >= 0; --ld)
+                    for (int lb = LMAX; lb >= 0; --lb) {
+                        const int lc = L - la - ld - lb;
+                        if (lc < 0 || lc > LMAX) continue;
                         if (h->nkblk[la][ld] <= 0 || !h->has_l[lb] || !h->has_l[lc]) continue;
                         const int cls = ((la * 3 + lb) * 3 + lc) * 3 + ld;
-                        if (h->profile) CK(cudaEventRecord(h->evK[cls][0], st));
-                        launch_sr_k(la, lb, lc, ld, sp, h->kblk[la][ld], h->nkblk[la][ld], st);
-                        if (h->profile) CK(cudaEventRecord(h->evK[cls][1], st));
+                        cudaStream_t cs = st;
+                        if (prof) CK(cudaEventRecord(h->evK[cls][0], cs));
+                        launch_sr_k(la, lb, lc, ld, h->mixed, sp, h->kblk[la][ld], h->nkblk[la][ld], cs);
+                        if (h->debug_sync) {
+                            const cudaError_t e = cudaStreamSynchronize(cs);
+                            if (e != cudaSuccess) {
+                                char buf[160];
+                                std::snprintf(buf, sizeof buf, "real-space K class (%d%d|%d%d): %s", la, lb, lc, ld, cudaGetErrorString(e));
+                                return fail(h, PBC_JK_ERR_CUDA, buf);
+                            }
+                        }
+                        if (prof) CK(cudaEventRecord(h->evK[cls][1], cs));
                         h->ranK[cls] = true;
                         ++nl;
                     }
     }
+    CK(cudaEventRecord(h->ev[2], st));
+    if (J && doSR) {
+        for (int LB = 4; LB >= 0; --LB) {
+            cudaStream_t cs = st;
+            for (int LK = 4; LK >= 0; --LK) {
+                if (h->njbra[LB] <= 0 || h->njbra[LK] <= 0) continue;
+                const int cls = LB * 5 + LK;
+                if (prof) CK(cudaEventRecord(h->evJ[cls][0], cs));
+                launch_sr_j(LB, LK, sp, h->jbra[LB], h->njbra[LB], cs);
+                if (h->debug_sync) {
+                    const cudaError_t e = cudaStreamSynchronize(cs);
+                    if (e != cudaSuccess) {
+                        char buf[160];
+                        std::snprintf(buf, sizeof buf, "real-space J class (%d,%d): %s", LB, LK, cudaGetErrorString(e));
+                        return fail(h, PBC_JK_ERR_CUDA, buf);
+                    }
+                }
+                if (prof) CK(cudaEventRecord(h->evJ[cls][1], cs));
+                h->ranJ[cls] = true;
+                ++nl;
+            }
+        }
+    }
     CK(cudaEventRecord(h->ev[3], st));
-    // ---- A7/A8: reciprocal space, batches of G ----
+    // ---- A7/A8: reciprocal space, batches of G (on the caller's stream) ----
     const bool needJlr = J && (doLR || doSELF), needKlr = K && (doLR || doSELF);
-    if (needJlr) CK(cudaMemsetAsync(h->Jlr, 0, NN * 8, st));
-    if (needKlr) CK(cudaMemsetAsync(h->Klr, 0, (size_t)h->nsplit * Np * Np * 8, st));
+    if (J) CK(cudaMemsetAsync(h->Jlr, 0, NN * 8, st));
+    if (K) CK(cudaMemsetAsync(h->Klr, 0, (size_t)h->nsplit * Np * Np * 8, st));
     const size_t strideK = (size_t)Np * Np;
     // K^LR = sum_slots Y^T Y with Y = L^T A', P' = L L^T (device-side rank; dense fallback inside the same kernels)
     if (needKlr) {
@@ -753,8 +943,11 @@ int pbc_jk_build(pbc_jk *h, const double *P, double *J, double *K, void *cuda_st
     }
     // one batch of S slots (layout A'[row*Np*S + col*S + slot]):  Y = L^T A'  (rows >= rank skipped), then
     // K += alpha sum_r sum_slot Y[r][mu][slot] Y[r][nu][slot] on the lower tiles (batches = rows r of the factor)
+    h->n_evG = 0;
     auto klr_batch = [&](int S, double alpha, int nsplit) {
         const size_t ldS = (size_t)Np * S;
+        const bool tg = prof && 2 * (size_t)h->n_evG + 1 < h->evG.size();
+        if (tg) cudaEventRecord(h->evG[2 * h->n_evG], st);
         GemmArgs g1;
         g1.M = Np; g1.Nc = Np * S; g1.Kb = Np; g1.nbatch = 1; g1.A = h->LT; g1.lda = Np; g1.B = h->Astack; g1.ldb = ldS;
         g1.C = h->Zstack; g1.ldc = ldS; g1.dyn = h->chol_dyn; g1.use_dyn = 1;
@@ -765,6 +958,7 @@ int pbc_jk_build(pbc_jk *h, const double *P, double *J, double *K, void *cuda_st
         g2.B_alt = h->Astack; g2.beta = 1.0; g2.C = h->Klr; g2.ldc = Np; g2.strideC = strideK; g2.nsplit = nsplit;
         g2.dyn = h->chol_dyn; g2.use_dyn = 4 | 8; g2.lower_only = 1;
         launch_dgemm(g2, st);
+        if (tg) { cudaEventRecord(h->evG[2 * h->n_evG + 1], st); ++h->n_evG; }
     };
     const int n_agen = agen_launches(h->lr);
     // Elements of shell pairs with no primitive pair-image are never written by agen_kernel and must read as 0:
@@ -775,7 +969,9 @@ int pbc_jk_build(pbc_jk *h, const double *P, double *J, double *K, void *cuda_st
         return cudaMemsetAsync(h->Astack, 0, (size_t)Np * Np * S * sizeof(double), st);
     };
     if (doLR) {
-        for (int g0 = 0; g0 < h->nG; g0 += h->nb) {
+        int ibatch = 0;
+        for (int g0 = 0; g0 < h->nG; g0 += h->nb, ++ibatch) {
+            if (ibatch % h->shard_n != h->shard_rank) continue;      // multi-GPU: G batches dealt round-robin
             const int nb = std::min(h->nb, h->nG - g0), S = ((2 * nb + 15) / 16) * 16;
             CK(set_layout(S));
             launch_agen(h->lr, g0, nb, S, 0.0, h->Astack, st);
@@ -799,10 +995,14 @@ int pbc_jk_build(pbc_jk *h, const double *P, double *J, double *K, void *cuda_st
         if (K) klr_batch(16, -1.0, h->nsplit);
     }
     CK(cudaEventRecord(h->ev[4], st));
+    if (J && doSR && h->U.nsp > 0) {
+        launch_j_backtransform(h->U, h->sh, h->Jt, h->Jsr, N, st);
+        ++nl;
+    }
     // ---- A10 ----
-    if (J) launch_finalize_j(doSR ? h->Jsr : nullptr, needJlr ? h->Jlr : nullptr, N, h->fcomp, J, st);
+    if (J) launch_finalize_j(doSR ? h->Jsr : nullptr, h->Jlr, N, h->fcomp, J, st);
     if (K)
-        launch_finalize_k(doSR ? h->Ksr : nullptr, h->sh, needKlr ? h->Klr : nullptr, h->nsplit, strideK, Np, N, h->fcomp,
+        launch_finalize_k(doSR ? h->Ksr : nullptr, h->sh, h->Klr, h->nsplit, strideK, Np, N, h->fcomp,
                           h->shell_of_ao, K, st);
     nl += (J ? 1 : 0) + (K ? 1 : 0);
     CK(cudaEventRecord(h->ev[5], st));
@@ -810,6 +1010,7 @@ int pbc_jk_build(pbc_jk *h, const double *P, double *J, double *K, void *cuda_st
     h->n_launches = nl;
     h->last_stream = st;
     h->built = true;
+    h->profiled_last = prof;
     return PBC_JK_OK;
 }
 
@@ -823,7 +1024,10 @@ int pbc_jk_build_host(pbc_jk *h, const double *P_host, double *J_host, double *K
     if (rc != PBC_JK_OK) return rc;
     if (J_host) CK(cudaMemcpyAsync(J_host, h->hostJ, bytes, cudaMemcpyDeviceToHost, 0));
     if (K_host) CK(cudaMemcpyAsync(K_host, h->hostK, bytes, cudaMemcpyDeviceToHost, 0));
+    unsigned long long flag = 0;
+    CK(cudaMemcpyAsync(&flag, h->counters + CNT_FLAG, sizeof(flag), cudaMemcpyDeviceToHost, 0));
     CK(cudaStreamSynchronize(0));
+    if (flag) return fail(h, PBC_JK_ERR_UNSUPPORTED, "max |P| exceeds 1e6: the lattice image range of the real-space sums was not validated for it");
     return PBC_JK_OK;
 }
 
@@ -839,13 +1043,29 @@ int pbc_jk_get_stats(pbc_jk *h, pbc_jk_stats_t *out)
         unsigned long long c[CNT_N];
         CK(cudaMemcpy(c, h->counters, sizeof(c), cudaMemcpyDeviceToHost));
         for (int i = 0; i < NCLS_J; ++i) { out->candidates_j += (int64_t)c[CNT_CAND_J + i]; out->quartets_j += (int64_t)c[CNT_Q_J + i]; }
-        for (int i = 0; i < NCLS_K; ++i) { out->candidates_k += (int64_t)c[CNT_CAND_K + i]; out->quartets_k += (int64_t)c[CNT_Q_K + i]; }
+        for (int i = 0; i < NCLS_K; ++i) {
+            out->candidates_k += (int64_t)c[CNT_CAND_K + i];
+            out->quartets_k += (int64_t)c[CNT_Q_K + i];
+            out->quartets_k_fp32 += (int64_t)c[CNT_Q32_K + i];
+        }
         out->n_launches = h->n_launches;
         float ms[5];
         for (int i = 0; i < 5; ++i) CK(cudaEventElapsedTime(&ms[i], h->ev[i], h->ev[i + 1]));
         float tot;
         CK(cudaEventElapsedTime(&tot, h->ev[0], h->ev[5]));
-        out->ms_density = ms[0]; out->ms_sr_j = ms[1]; out->ms_sr_k = ms[2]; out->ms_lr = ms[3] + ms[4]; out->ms_total = tot;
+        out->ms_density = ms[0]; out->ms_sr_k = ms[1]; out->ms_sr_j = ms[2]; out->ms_lr = ms[3] + ms[4]; out->ms_total = tot;
+        if (h->profiled_last)
+            for (int i = 0; i < h->n_evG; ++i) {
+                float t = 0.f;
+                CK(cudaEventElapsedTime(&t, h->evG[2 * i], h->evG[2 * i + 1]));
+                out->ms_lr_gemm += t;
+            }
+        {
+            int dyn[2] = {0, 0};
+            CK(cudaMemcpy(dyn, h->chol_dyn, sizeof(dyn), cudaMemcpyDeviceToHost));
+            out->rank_p = dyn[0];
+        }
+        if (c[CNT_FLAG]) return fail(h, PBC_JK_ERR_UNSUPPORTED, "max |P| exceeds 1e6: the lattice image range of the real-space sums was not validated for it");
     }
     return PBC_JK_OK;
 }
@@ -873,7 +1093,7 @@ int pbc_jk_get_class_stats(pbc_jk *h, pbc_jk_class_stat *out, int32_t cap, int32
             s.kind = 0; s.l[0] = cls / 5; s.l[1] = cls % 5; s.l[2] = s.l[3] = 0;
             s.quartets = (int64_t)c[CNT_Q_J + cls]; s.candidates = (int64_t)c[CNT_CAND_J + cls];
             float ms = 0.f;
-            if (h->profile) CK(cudaEventElapsedTime(&ms, h->evJ[cls][0], h->evJ[cls][1]));
+            if (h->profiled_last) CK(cudaEventElapsedTime(&ms, h->evJ[cls][0], h->evJ[cls][1]));
             s.ms = ms;
         }
         ++n;
@@ -885,7 +1105,7 @@ int pbc_jk_get_class_stats(pbc_jk *h, pbc_jk_class_stat *out, int32_t cap, int32
             s.kind = 1; s.l[0] = cls / 27; s.l[1] = (cls / 9) % 3; s.l[2] = (cls / 3) % 3; s.l[3] = cls % 3;
             s.quartets = (int64_t)c[CNT_Q_K + cls]; s.candidates = (int64_t)c[CNT_CAND_K + cls];
             float ms = 0.f;
-            if (h->profile) CK(cudaEventElapsedTime(&ms, h->evK[cls][0], h->evK[cls][1]));
+            if (h->profiled_last) CK(cudaEventElapsedTime(&ms, h->evK[cls][0], h->evK[cls][1]));
             s.ms = ms;
         }
         ++n;
@@ -903,20 +1123,6 @@ int pbc_jk_destroy(pbc_jk *h)
     h->pool.free_all();
     destroy_events(h);
     delete h;
-    return PBC_JK_OK;
-}
-
-int pbc_jk_fp64_peak(int32_t iters, double *tflops_out)
-{
-    if (!tflops_out || iters < 1) return PBC_JK_ERR_INVALID_ARG;
-    int ndev = 0;
-    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
-        cudaGetLastError();
-        return PBC_JK_ERR_CUDA;
-    }
-    const double v = run_fp64_peak(iters);
-    if (v < 0) return PBC_JK_ERR_CUDA;
-    *tflops_out = v;
     return PBC_JK_OK;
 }
 

@@ -15,8 +15,8 @@
 namespace pbcjk {
 
 // ---------------------------------------------------------------- density prep (A4)
-__global__ void scale_density_kernel(const double *__restrict__ P, double *__restrict__ Pp, int N, int Np,
-                                     const double *__restrict__ f, unsigned long long *maxbits)
+__global__ void scale_density_kernel(const double *__restrict__ P, double *__restrict__ Pp, float *__restrict__ Ppf, int N,
+                                     int Np, const double *__restrict__ f, unsigned long long *maxbits)
 {
     const size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     double v = 0.0;
@@ -24,6 +24,7 @@ __global__ void scale_density_kernel(const double *__restrict__ P, double *__res
         const int i = (int)(idx / N), j = (int)(idx % N);
         v = P[idx] * f[i] * f[j];
         Pp[(size_t)i * Np + j] = v;
+        if (Ppf) Ppf[(size_t)i * Np + j] = (float)v;
         v = fabs(v);
     }
     // block maximum; one atomic per block (not on the quartet path)
@@ -38,18 +39,73 @@ __global__ void scale_density_kernel(const double *__restrict__ P, double *__res
         atomicMax(maxbits, (unsigned long long)__double_as_longlong(m));
     }
 }
-__global__ void lnpmax_kernel(const unsigned long long *maxbits, double *lnPmax)
+__global__ void lnpmax_kernel(const unsigned long long *maxbits, double *lnPmax, unsigned long long *flag)
 {
     double m = __longlong_as_double((long long)*maxbits);
     *lnPmax = log(fmax(m, 1e-300));
+    // the lattice image range of the real-space scans was validated at create for max|P'| <= e^{LN_PMAX_CAP}
+    if (*lnPmax > LN_PMAX_CAP) *flag = 1ull;
 }
-void launch_scale_density(const double *P, double *Pp, int N, int Np, const double *fcomp,
-                          unsigned long long *maxbits, double *lnPmax, cudaStream_t st)
+void launch_scale_density(const double *P, double *Pp, float *Ppf, int N, int Np, const double *fcomp,
+                          unsigned long long *maxbits, double *lnPmax, unsigned long long *flag, cudaStream_t st)
 {
     cudaMemsetAsync(maxbits, 0, sizeof(unsigned long long), st);
     const size_t tot = (size_t)N * N;
-    scale_density_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, st>>>(P, Pp, N, Np, fcomp, maxbits);
-    lnpmax_kernel<<<1, 1, 0, st>>>(maxbits, lnPmax);
+    scale_density_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, st>>>(P, Pp, Ppf, N, Np, fcomp, maxbits);
+    lnpmax_kernel<<<1, 1, 0, st>>>(maxbits, lnPmax, flag);
+}
+
+// ln(max |P'|) over every shell block (lambda, sigma) and its row maxima: the density-weighted screen
+__global__ void density_blocks_kernel(const double *__restrict__ Pp, int Np, ShellInfo sh, float *__restrict__ lnPblk)
+{
+    const int b = blockIdx.x * blockDim.x + threadIdx.x, a = blockIdx.y;
+    if (b >= sh.nshell) return;
+    const int na = ncart(sh.l[a]), nb = ncart(sh.l[b]);
+    const double *blk = Pp + (size_t)sh.ao[a] * Np + sh.ao[b];
+    double m = 0.0;
+    for (int i = 0; i < na; ++i)
+        for (int j = 0; j < nb; ++j) m = fmax(m, fabs(blk[(size_t)i * Np + j]));
+    // rounded up a little so that the fp32 value never undercuts the fp64 maximum
+    lnPblk[(size_t)a * sh.nshell + b] = m > 0.0 ? (float)log(m) + 1e-5f : -200.f;
+}
+__global__ void density_rows_kernel(const float *__restrict__ lnPblk, int ns, float *__restrict__ lnProw)
+{
+    const int a = blockIdx.x;
+    float m = -200.f;
+    for (int b = threadIdx.x; b < ns; b += blockDim.x) m = fmaxf(m, lnPblk[(size_t)a * ns + b]);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, o));
+    __shared__ float s[8];
+    if ((threadIdx.x & 31) == 0) s[threadIdx.x >> 5] = m;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        for (int w = 1; w < (int)(blockDim.x >> 5); ++w) m = fmaxf(m, s[w]);
+        lnProw[a] = m;
+    }
+}
+__global__ void ket_density_kernel(const float *__restrict__ lnPblk, int ns, KetListJ KJ, float *__restrict__ kjP)
+{
+    const int j = blockIdx.x * blockDim.x + threadIdx.x;
+    if (j < KJ.n) kjP[j] = lnPblk[(size_t)KJ.spA[j] * ns + KJ.spB[j]];
+}
+void launch_density_blocks(const double *Pp, int Np, const ShellInfo &sh, const KetListJ &KJ, float *lnPblk, float *lnProw,
+                           float *kjP, cudaStream_t st)
+{
+    dim3 grid((sh.nshell + 127) / 128, sh.nshell);
+    density_blocks_kernel<<<grid, 128, 0, st>>>(Pp, Np, sh, lnPblk);
+    density_rows_kernel<<<sh.nshell, 256, 0, st>>>(lnPblk, sh.nshell, lnProw);
+    if (KJ.n > 0) ket_density_kernel<<<(KJ.n + 255) / 256, 256, 0, st>>>(lnPblk, sh.nshell, KJ, kjP);
+}
+
+__global__ void to_float_kernel(const double *__restrict__ src, float *__restrict__ dst, size_t n)
+{
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) dst[i] = (float)src[i];
+}
+void launch_to_float(const double *src, float *dst, size_t n, cudaStream_t st)
+{
+    if (n == 0) return;
+    to_float_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(src, dst, n);
 }
 
 // Hermite density of a ket primitive pair-image: D~_s = fac * sum_{cd} E^{cd}_s P'_cd   (eq 95)
@@ -506,17 +562,19 @@ __global__ void __launch_bounds__(256) dgemm_kernel(int Kb, int nbatch, double a
         }
 }
 
+namespace {
+constexpr int smemN = 2 * (BM * SA + BK * SB) * (int)sizeof(double), smemT = 2 * (2 * BK * SB) * (int)sizeof(double);
+constexpr int smemNT = 2 * (BM * SA + BN * SA) * (int)sizeof(double);
+}  // namespace
+// the opt-in is per device: pbc_jk_create calls this for the handle's device
+void dgemm_set_attributes()
+{
+    cudaFuncSetAttribute(dgemm_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smemN);
+    cudaFuncSetAttribute(dgemm_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smemT);
+    cudaFuncSetAttribute(dgemm_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smemNT);
+}
 void launch_dgemm(const GemmArgs &g, cudaStream_t st)
 {
-    static bool attr_set = false;
-    constexpr int smemN = 2 * (BM * SA + BK * SB) * (int)sizeof(double), smemT = 2 * (2 * BK * SB) * (int)sizeof(double);
-    constexpr int smemNT = 2 * (BM * SA + BN * SA) * (int)sizeof(double);
-    if (!attr_set) {
-        cudaFuncSetAttribute(dgemm_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smemN);
-        cudaFuncSetAttribute(dgemm_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smemT);
-        cudaFuncSetAttribute(dgemm_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smemNT);
-        attr_set = true;
-    }
     dim3 grid(g.Nc / BN, g.M / BM, g.nsplit);
     if (g.transA)
         dgemm_kernel<true, false><<<grid, 256, smemT, st>>>(g.Kb, g.nbatch, g.alpha, g.A, g.lda, g.strideA, g.B, g.ldb, g.strideB,
@@ -719,45 +777,6 @@ void launch_extract_overlap(const double *Astack, int Np, int S, int N, const do
 {
     dim3 grid((N + 127) / 128, N);
     extract_overlap_kernel<<<grid, 128, 0, st>>>(Astack, (size_t)Np * S, S, N, fcomp, Sm);
-}
-
-// ---------------------------------------------------------------- FP64 FMA peak (roofline denominator)
-__global__ void __launch_bounds__(256) fp64_peak_kernel(int iters, double *out)
-{
-    double a0 = threadIdx.x * 1e-9, a1 = a0 + 1, a2 = a0 + 2, a3 = a0 + 3, a4 = a0 + 4, a5 = a0 + 5, a6 = a0 + 6, a7 = a0 + 7;
-    const double b = 1.0000001, c = 1e-9;
-    for (int i = 0; i < iters; ++i) {
-#pragma unroll
-        for (int k = 0; k < 8; ++k) {
-            a0 = fma(a0, b, c); a1 = fma(a1, b, c); a2 = fma(a2, b, c); a3 = fma(a3, b, c);
-            a4 = fma(a4, b, c); a5 = fma(a5, b, c); a6 = fma(a6, b, c); a7 = fma(a7, b, c);
-        }
-    }
-    const double s = a0 + a1 + a2 + a3 + a4 + a5 + a6 + a7;
-    if (s == 1.2345) out[0] = s;
-}
-double run_fp64_peak(int iters)
-{
-    int dev = 0, nsm = 0;
-    cudaGetDevice(&dev);
-    cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
-    double *d = nullptr;
-    if (cudaMalloc(&d, 8) != cudaSuccess) return -1.0;
-    cudaEvent_t e0, e1;
-    cudaEventCreate(&e0); cudaEventCreate(&e1);
-    const int blocks = nsm * 8;
-    fp64_peak_kernel<<<blocks, 256>>>(iters / 8 + 1, d);
-    cudaEventRecord(e0);
-    fp64_peak_kernel<<<blocks, 256>>>(iters, d);
-    cudaEventRecord(e1);
-    cudaEventSynchronize(e1);
-    float ms = 0;
-    cudaEventElapsedTime(&ms, e0, e1);
-    cudaEventDestroy(e0); cudaEventDestroy(e1);
-    cudaFree(d);
-    if (cudaGetLastError() != cudaSuccess || ms <= 0) return -1.0;
-    const double flop = 2.0 * 64.0 * (double)iters * 256.0 * blocks;
-    return flop / (ms * 1e-3) * 1e-12;
 }
 
 }  // namespace pbcjk

@@ -17,8 +17,14 @@ struct LRParams {
 };
 
 // P' = f P f (into the padded Np x Np buffer, pads untouched) and ln(max |P'|)
-void launch_scale_density(const double *P, double *Pp, int N, int Np, const double *fcomp,
-                          unsigned long long *maxbits, double *lnPmax, cudaStream_t st);
+// (Ppf: optional fp32 copy for the mixed-precision evaluators; flag: set when max|P'| exceeds e^{LN_PMAX_CAP})
+void launch_scale_density(const double *P, double *Pp, float *Ppf, int N, int Np, const double *fcomp,
+                          unsigned long long *maxbits, double *lnPmax, unsigned long long *flag, cudaStream_t st);
+// ln max|P'| per shell block [nshell x nshell], its row maxima, and the block value of every J ket's own pair (L819)
+void launch_density_blocks(const double *Pp, int Np, const ShellInfo &sh, const KetListJ &KJ, float *lnPblk, float *lnProw,
+                           float *kjP, cudaStream_t st);
+void launch_to_float(const double *src, float *dst, size_t n, cudaStream_t st);
+void dgemm_set_attributes();
 // E^{AB}_t product table of the ordered pair list (rows at K.eoff), built once per geometry
 void launch_etab(const PairListK &K, const int *lA, const int *lB, double *etab, cudaStream_t st);
 // D~_s of every J ket (eq 95)
@@ -64,6 +70,5 @@ void launch_finalize_j(const double *Jsr, const double *Jlr, int N, const double
 void launch_finalize_k(const double *Ksr, const ShellInfo &sh, const double *Klr, int nsplit, size_t strideK, int Np,
                        int N, const double *fcomp, const int *shell_of_ao, double *K, cudaStream_t st);
 void launch_extract_overlap(const double *Astack, int Np, int S, int N, const double *fcomp, double *Sm, cudaStream_t st);
-double run_fp64_peak(int iters);
 
 }  // namespace pbcjk

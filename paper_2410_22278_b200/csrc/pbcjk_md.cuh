@@ -1,5 +1,5 @@
 // McMurchie-Davidson building blocks for the real-space (erfc) quartet kernels.
-//   Boys F_m: tabulated, Taylor + downward recursion (eq 28 L209 is m = 0; split eq 30)
+//   Boys F_m: tabulated Taylor coefficients + downward recursion (eq 28 L209 is m = 0; split eq 30)
 //   merged base values R^m_000 = (-2 alpha)^m F_m(alpha r^2) - theta (-2 alpha_w)^m F_m(alpha_w r^2)
 //     (eq 50 L362 applied to both terms of eq 56; merged BEFORE the recursion because eq 47-49
 //      depend only on the separation vector)
@@ -11,50 +11,99 @@
 
 namespace pbcjk {
 
-// F_0..F_L at x.  tab: BOYS_ROWS x BOYS_MCOL, tab[i][m] = F_m(i*BOYS_DX).
+// Boys tables (built on the host at create, pbcjk_api.cu):
+//   c  [LTOT+1][BOYS_ROWS][8]: Taylor coefficients of F_L around the grid point x_i = i*BOYS_DX,
+//        c[L][i][k] = F_{L+k}(x_i)/k!   (d/dx F_m = -F_{m+1}), so F_L(x) = sum_k c_k (x_i - x)^k   (Horner, 7 FMA);
+//        one row = one 64-byte line, read as four 16-byte loads
+//   ex [BOYS_ROWS]: exp(-x_i); exp(-x) = exp(-x_i) exp(x_i - x) with a degree-8 Taylor polynomial (|x_i - x| <= 1/16:
+//        truncation 4e-17) instead of a double-precision exp() call
+//   cf, exf: fp32 copies for the mixed-precision evaluators
+struct BoysTab {
+    const double *c, *ex;
+    const float *cf;
+};
+
+// F_0..F_L at x: Taylor expansion of the top order around the nearest grid point, downward recursion
+// F_{m-1} = (2x F_m + e^{-x})/(2m-1); asymptotic form beyond BOYS_XMAX.
 template <int L>
-__device__ __forceinline__ void boys(const double *__restrict__ tab, double x, double *F)
+__device__ __forceinline__ void boys(const BoysTab &tb, double x, double *F)
 {
     if (x < BOYS_XMAX) {
-        int i = __double2int_rn(x * (1.0 / BOYS_DX));
-        double dx = fma((double)i, BOYS_DX, -x);                 // x0 - x, |dx| <= 1/16
-        const double *row = tab + i * BOYS_MCOL + L;
-        // F_L(x) = sum_k F_{L+k}(x0) dx^k / k!   (d/dx F_m = -F_{m+1}), nested form
-        double f = __ldg(row + 7);
-        f = fma(f, dx * (1.0 / 7.0), __ldg(row + 6));
-        f = fma(f, dx * (1.0 / 6.0), __ldg(row + 5));
-        f = fma(f, dx * (1.0 / 5.0), __ldg(row + 4));
-        f = fma(f, dx * (1.0 / 4.0), __ldg(row + 3));
-        f = fma(f, dx * (1.0 / 3.0), __ldg(row + 2));
-        f = fma(f, dx * 0.5, __ldg(row + 1));
-        f = fma(f, dx, __ldg(row));
+        const int i = __double2int_rn(x * (1.0 / BOYS_DX));
+        const double dx = fma((double)i, BOYS_DX, -x);                 // x_i - x, |dx| <= 1/16
+        const double2 *row = reinterpret_cast<const double2 *>(tb.c + ((size_t)L * BOYS_ROWS + i) * 8);
+        const double2 c01 = __ldg(row), c23 = __ldg(row + 1), c45 = __ldg(row + 2), c67 = __ldg(row + 3);
+        double f = fma(c67.y, dx, c67.x);
+        f = fma(f, dx, c45.y);
+        f = fma(f, dx, c45.x);
+        f = fma(f, dx, c23.y);
+        f = fma(f, dx, c23.x);
+        f = fma(f, dx, c01.y);
+        f = fma(f, dx, c01.x);
         F[L] = f;
         if (L > 0) {
-            double ex = exp(-x);
-            double x2 = x + x;
+            double e = fma(1.0 / 40320.0, dx, 1.0 / 5040.0);
+            e = fma(e, dx, 1.0 / 720.0);
+            e = fma(e, dx, 1.0 / 120.0);
+            e = fma(e, dx, 1.0 / 24.0);
+            e = fma(e, dx, 1.0 / 6.0);
+            e = fma(e, dx, 0.5);
+            e = fma(e, dx, 1.0);
+            e = fma(e, dx, 1.0);
+            const double ex = __ldg(tb.ex + i) * e;
+            const double x2 = x + x;
 #pragma unroll
             for (int m = L; m > 0; --m) F[m - 1] = fma(x2, F[m], ex) * (1.0 / (2.0 * m - 1.0));
         }
     } else {
         // F_0 = sqrt(pi/x)/2 up to e^-x (< 3e-16 here); F_{m+1} = (2m+1) F_m / (2x)
-        double rs = rsqrt(x);
-        double ix = rs * rs;
+        const double rs = rsqrt(x);
+        const double ix = rs * rs;
         F[0] = 0.88622692545275801365 * rs;
 #pragma unroll
         for (int m = 0; m < L; ++m) F[m + 1] = F[m] * ((m + 0.5) * ix);
     }
 }
 
-// Rm[m] = pref * [ (-2 alpha)^m F_m(alpha r2) - theta (-2 alpha_w)^m F_m(alpha_w r2) ],  m = 0..L
+// fp32 variant (mixed precision, PAPER 3.5 L817): degree-5 Taylor (|dx|^6/720 < 1e-10), fast exp
 template <int L>
-__device__ __forceinline__ void boys_merged(const double *__restrict__ tab, double r2, double alpha,
-                                            double alpha_w, double theta, double pref, double *Rm)
+__device__ __forceinline__ void boys(const BoysTab &tb, float x, float *F)
 {
-    double F1[L + 1], F2[L + 1];
-    boys<L>(tab, alpha * r2, F1);
-    boys<L>(tab, alpha_w * r2, F2);
-    double c1 = pref, c2 = -pref * theta;
-    double m2a = -2.0 * alpha, m2w = -2.0 * alpha_w;
+    if (x < (float)BOYS_XMAX) {
+        const int i = __float2int_rn(x * (float)(1.0 / BOYS_DX));
+        const float dx = fmaf((float)i, (float)BOYS_DX, -x);
+        const float4 *row = reinterpret_cast<const float4 *>(tb.cf + ((size_t)L * BOYS_ROWS + i) * 8);
+        const float4 c03 = __ldg(row), c47 = __ldg(row + 1);
+        float f = fmaf(c47.y, dx, c47.x);
+        f = fmaf(f, dx, c03.w);
+        f = fmaf(f, dx, c03.z);
+        f = fmaf(f, dx, c03.y);
+        f = fmaf(f, dx, c03.x);
+        F[L] = f;
+        if (L > 0) {
+            const float ex = __expf(-x);
+            const float x2 = x + x;
+#pragma unroll
+            for (int m = L; m > 0; --m) F[m - 1] = fmaf(x2, F[m], ex) * (1.0f / (2.0f * m - 1.0f));
+        }
+    } else {
+        const float rs = rsqrtf(x);
+        const float ix = rs * rs;
+        F[0] = 0.886226925f * rs;
+#pragma unroll
+        for (int m = 0; m < L; ++m) F[m + 1] = F[m] * ((m + 0.5f) * ix);
+    }
+}
+
+// Rm[m] = pref * [ (-2 alpha)^m F_m(alpha r2) - theta (-2 alpha_w)^m F_m(alpha_w r2) ],  m = 0..L
+template <int L, typename T>
+__device__ __forceinline__ void boys_merged(const BoysTab &tb, T r2, T alpha, T alpha_w, T theta, T pref, T *Rm)
+{
+    T F1[L + 1], F2[L + 1];
+    boys<L>(tb, alpha * r2, F1);
+    boys<L>(tb, alpha_w * r2, F2);
+    T c1 = pref, c2 = -pref * theta;
+    const T m2a = T(-2.0) * alpha, m2w = T(-2.0) * alpha_w;
 #pragma unroll
     for (int m = 0; m <= L; ++m) {
         Rm[m] = fma(c1, F1[m], c2 * F2[m]);

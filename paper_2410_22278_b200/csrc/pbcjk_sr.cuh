@@ -2,16 +2,22 @@
 // eq 56/69).  One kernel family per angular-momentum class, generated from templates.
 //
 // Mapping (differs from PAPER 3.2 L753, which gives one THREAD a bra pair and lets it loop over
-// its own lattice sphere -> warp divergence, L882):
-//   * one WARP owns one bra primitive pair-image; its data are warp-uniform.
-//   * phase 1 (cheap, divergent): lanes stream over the ket primitive pair-images of a group
-//     (sorted by bound, so the loop ends early) for every lattice image R1 in the bounding box of
-//     eq 99-103, test the eq-67 bound per (ket, R1) and push survivors into a per-warp
-//     shared-memory queue (ballot + popc compaction).
-//   * phase 2 (expensive, convergent): whenever 32 survivors are queued, every lane evaluates one
-//     primitive quartet-image: merged Boys values, Hermite R recursion, contraction.
-//   * accumulators stay in registers; warp-shuffle + shared-memory reductions; every output
-//     element has exactly one owner, so there are no global atomics on the data path.
+// its own lattice sphere -> warp divergence, L882).  Both families run a two-level screen in front
+// of a convergent evaluator:
+//   * level A (lane-parallel, fp32): an ITEM is a (ket group, lattice image) pair for the J-engine
+//     (the warp owns one bra) or a (bra, lattice image) pair for K (the CTA owns one ket group).  32
+//     items are screened at a time, one per lane: distance of the bra centre to the translated group
+//     centre, the bound `need` a ket of that group must exceed there (eq 67 at the closest approach),
+//     and -- the kets of a group being sorted by bound -- the NUMBER of kets that exceed it, by binary
+//     search.  Items with a zero count cost nothing further.
+//   * level B: for every live item (ballot + shuffle broadcast) the lanes test its kets, 32 at a time, with the eq-67 screen in fp32 on 16-byte screen records (positions relative to the group
+//     centre), then with the per-shell-block max |P| (L819); survivors go to a per-warp ring in shared
+//     memory (ballot + popc compaction).
+//   * evaluation (expensive, convergent, fp64): whenever 32 survivors are queued every lane evaluates
+//     one primitive quartet-image: merged Boys values, Hermite R recursion, contraction.
+//   * accumulators stay in registers; warp-shuffle + shared-memory reductions; every output element
+//     has exactly one owner, so there are no global atomics on the data path.
+// The fp32 screen keeps a superset of the fp64 rule (slack SCREEN_MARGIN in the logarithm of the bound).
 #pragma once
 #include "pbcjk_md.cuh"
 
@@ -23,123 +29,79 @@ struct SRParams {
     KetListJ KJ;
     Lattice lat;
     ShellInfo sh;
-    const double *boys;
+    BoysTab boys;
     const double *Pp;        // P with component factors folded in, row stride ldP
+    const float *Ppf;        // fp32 copy of P' (mixed precision), same stride
     int ldP;
     const double *Dt;        // Hermite densities of the J kets, Dt[s*dstride + j]   (eq 95)
     double *Jt;              // Hermite J of the U entries, Jt[t*U.n + u]            (eq 98, raw)
     double *Ksr;             // N x N, accumulated block by block
     const double *lnPmax;    // device scalar ln(max |P'|)
+    const float *lnPblk;     // [nshell*nshell] ln(max |P'|) over each shell block (L819)
+    const float *lnProw;     // [nshell] row maxima of lnPblk
+    const float *kjP;        // [KJ.n] lnPblk of each J ket's own shell pair
     double ln_tau;           // ln(d_schwarz)
     double rcut2;            // r_cut^2 (C-14) or +inf
+    float ln_switch;         // mixed precision: ln(mixed_switch); quartets whose ln(bound_bra bound_ket max|P block|)
+                             // is below it are evaluated in fp32 (PAPER 3.5 L819)
+    int shard_rank, shard_n; // multi-GPU: this rank takes blocks / bras with index % shard_n == shard_rank
     unsigned long long *counters;
 };
 
-constexpr int QCAP = 64;
+constexpr int QCAP = 64;        // survivor ring per warp (power of two)
+constexpr int NIMG_J = 64;      // lattice images per warp-level list chunk (J-engine)
 
-__device__ __forceinline__ int pack_img(int n0, int n1, int n2)
+__device__ __forceinline__ void lattice_T(const Lattice &lat, int n0, int n1, int n2, double &Tx, double &Ty, double &Tz)
 {
-    return ((n0 + 512) << 20) | ((n1 + 512) << 10) | (n2 + 512);
-}
-__device__ __forceinline__ void unpack_img(int t, const Lattice &lat, double &Tx, double &Ty, double &Tz)
-{
-    double n0 = (double)((t >> 20) - 512), n1 = (double)(((t >> 10) & 1023) - 512), n2 = (double)((t & 1023) - 512);
-    Tx = fma(n0, lat.a[0], fma(n1, lat.a[3], n2 * lat.a[6]));
-    Ty = fma(n0, lat.a[1], fma(n1, lat.a[4], n2 * lat.a[7]));
-    Tz = fma(n0, lat.a[2], fma(n1, lat.a[5], n2 * lat.a[8]));
+    Tx = n0 * lat.a[0] + n1 * lat.a[3] + n2 * lat.a[6];
+    Ty = n0 * lat.a[1] + n1 * lat.a[4] + n2 * lat.a[7];
+    Tz = n0 * lat.a[2] + n1 * lat.a[5] + n2 * lat.a[8];
 }
 
-// Phase 1 for one ket group [k0,k1) (sorted by lb descending) against the warp's bra, over all
-// lattice images within `rho` of the group centre (eq 99-103: bounding box, then sphere filter).
-// thr = lb_bra + ln(Pmax) - ln(tau); a (ket, image) survives iff
-//   thr + lb_ket - r^2/(1/p + 1/q + 1/w^2) > 0       (eq 67 with C_2e split per pair)
-template <class Eval>
-__device__ __forceinline__ void scan_group(const Lattice &lat, double Pix, double Piy, double Piz,
-                                           double ipi, double thr, double gx, double gy, double gz,
-                                           double ext, double iqmax, int k0, int k1,
-                                           const double *__restrict__ kQx, const double *__restrict__ kQy,
-                                           const double *__restrict__ kQz, const double *__restrict__ kiq,
-                                           const double *__restrict__ klb, double rcut2, int2 *queue,
-                                           int &qn, int lane, unsigned &ncand, unsigned &nq, Eval &&eval)
-{
-    if (k1 <= k0) return;
-    const double lbmax = __ldg(klb + k0);
-    const double budget = thr + lbmax;
-    if (budget <= 0.0) return;
-    const double isum_max = ipi + iqmax + lat.iomega2;
-    double rr = sqrt(budget * isum_max);
-    const double rho = rr + ext;
-    const double cx = Pix - gx, cy = Piy - gy, cz = Piz - gz;   // offset of the sphere centre
-    const double f0 = lat.binv[0] * cx + lat.binv[1] * cy + lat.binv[2] * cz;
-    const double f1 = lat.binv[3] * cx + lat.binv[4] * cy + lat.binv[5] * cz;
-    const double f2 = lat.binv[6] * cx + lat.binv[7] * cy + lat.binv[8] * cz;
-    const int lo0 = (int)ceil(f0 - rho * lat.bnorm[0]), hi0 = (int)floor(f0 + rho * lat.bnorm[0]);
-    const int lo1 = (int)ceil(f1 - rho * lat.bnorm[1]), hi1 = (int)floor(f1 + rho * lat.bnorm[1]);
-    const int lo2 = (int)ceil(f2 - rho * lat.bnorm[2]), hi2 = (int)floor(f2 + rho * lat.bnorm[2]);
-    const unsigned ltmask = (1u << lane) - 1u;
-    const int d1 = hi1 - lo1 + 1, d2 = hi2 - lo2 + 1, d12 = d1 * d2;
-    const int nimg = (hi0 >= lo0 && d1 > 0 && d2 > 0) ? (hi0 - lo0 + 1) * d12 : 0;
-    const double inv_isum_max = 1.0 / isum_max, rho2 = rho * rho;
-    for (int base = 0; base < nimg; base += 32) {
-        // 32 images of the box at a time, one per lane: sphere filter and the bound a ket needs there
-        const int im = base + lane;
-        bool ok = false;
-        double need_l = 0.0;
-        int timg_l = 0;
-        if (im < nimg) {
-            const int n0 = lo0 + im / d12, r = im % d12;
-            const int n1 = lo1 + r / d2, n2 = lo2 + r % d2;
-            const double Tx = n0 * lat.a[0] + n1 * lat.a[3] + n2 * lat.a[6];
-            const double Ty = n0 * lat.a[1] + n1 * lat.a[4] + n2 * lat.a[7];
-            const double Tz = n0 * lat.a[2] + n1 * lat.a[5] + n2 * lat.a[8];
-            const double ex = Tx - cx, ey = Ty - cy, ez = Tz - cz;
-            const double dist2 = ex * ex + ey * ey + ez * ez;
-            ok = dist2 <= rho2;
-            double dlb = sqrt(dist2) - ext;                     // lower bound of |Q + T - P|
-            dlb = dlb > 0.0 ? dlb : 0.0;
-            need_l = dlb * dlb * inv_isum_max - thr;            // ket survives only if lb_ket > need
-            timg_l = pack_img(n0, n1, n2);
-        }
-        unsigned imask = __ballot_sync(0xffffffffu, ok);
-        while (imask) {
-            const int src = __ffs(imask) - 1;
-            imask &= imask - 1;
-            const double need = __shfl_sync(0xffffffffu, need_l, src);
-            const int timg = __shfl_sync(0xffffffffu, timg_l, src);
-            double Tx, Ty, Tz;
-            unpack_img(timg, lat, Tx, Ty, Tz);
-            const double ox = Tx - Pix, oy = Ty - Piy, oz = Tz - Piz;
-            for (int j0 = k0; j0 < k1; j0 += 32) {
-                if (__ldg(klb + j0) <= need) break;             // sorted: nothing further survives
-                const int j = j0 + lane;
-                bool pass = false;
-                if (j < k1) {
-                    const double dx = __ldg(kQx + j) + ox, dy = __ldg(kQy + j) + oy, dz = __ldg(kQz + j) + oz;
-                    const double r2 = dx * dx + dy * dy + dz * dz;
-                    const double isum = ipi + __ldg(kiq + j) + lat.iomega2;
-                    pass = (thr + __ldg(klb + j)) * isum > r2 && r2 <= rcut2;
-                    ++ncand;
-                }
-                const unsigned m = __ballot_sync(0xffffffffu, pass);
-                if (pass) queue[qn + __popc(m & ltmask)] = make_int2(j, timg);
-                qn += __popc(m);
-                __syncwarp();
-                if (qn >= 32) {
-                    qn -= 32;
-                    const int2 e = queue[qn + lane];
-                    __syncwarp();
-                    eval(e.x, e.y);
-                    ++nq;
-                }
-            }
-        }
+// Bounding box (eq 99-103) of the lattice points within `rad` of the point c.
+struct ImageBox {
+    int lo0, lo1, lo2, d2, d12, n;
+    __device__ __forceinline__ void set(const Lattice &lat, double cx, double cy, double cz, double rad)
+    {
+        const double f0 = lat.binv[0] * cx + lat.binv[1] * cy + lat.binv[2] * cz;
+        const double f1 = lat.binv[3] * cx + lat.binv[4] * cy + lat.binv[5] * cz;
+        const double f2 = lat.binv[6] * cx + lat.binv[7] * cy + lat.binv[8] * cz;
+        lo0 = (int)ceil(f0 - rad * lat.bnorm[0]);
+        lo1 = (int)ceil(f1 - rad * lat.bnorm[1]);
+        lo2 = (int)ceil(f2 - rad * lat.bnorm[2]);
+        const int hi0 = (int)floor(f0 + rad * lat.bnorm[0]), hi1 = (int)floor(f1 + rad * lat.bnorm[1]);
+        const int hi2 = (int)floor(f2 + rad * lat.bnorm[2]);
+        const int d1 = hi1 - lo1 + 1;
+        d2 = hi2 - lo2 + 1;
+        d12 = d1 * d2;
+        n = (hi0 >= lo0 && d1 > 0 && d2 > 0) ? (hi0 - lo0 + 1) * d12 : 0;
     }
+    __device__ __forceinline__ void decode(int im, int &n0, int &n1, int &n2) const
+    {
+        n0 = lo0 + im / d12;
+        const int r = im % d12;
+        n1 = lo1 + r / d2;
+        n2 = lo2 + r % d2;
+    }
+};
+
+// number of leading entries of a list sorted by descending bound (q4[].w) that exceed `need` (per lane)
+__device__ __forceinline__ int count_above_sorted(const float4 *__restrict__ q4, int n, float need)
+{
+    int lo = 0, hi = n;
+    while (lo < hi) {
+        const int mid = (lo + hi) >> 1;
+        if (__ldg(&q4[mid].w) > need) lo = mid + 1;
+        else hi = mid;
+    }
+    return lo;
 }
 
 // ------------------------------------------------------------------------------------------
 // J-engine: bra Hermite order LB (= la+lb), ket Hermite order LK.  One warp per bra U entry.
 //   Jt[t] += sum_kets pref * sum_s R_{t+s}(Q - P + R1) D~_s        (eq 98 second term, reading C-4;
 //   the (-1)^{|t|} and E^{ab}_t are applied by the back-transform kernel, eq 97)
+// Ket groups: (atom of the ket's home shell, LK), sorted by bound; an item is (atom, lattice image).
 // ------------------------------------------------------------------------------------------
 template <int LB, int LK>
 __global__ void __launch_bounds__(128) sr_j_kernel(SRParams p, const int *__restrict__ bra_idx, int nbra)
@@ -147,72 +109,184 @@ __global__ void __launch_bounds__(128) sr_j_kernel(SRParams p, const int *__rest
     constexpr int L = LB + LK;
     constexpr int NT = nherm(LB), NS = nherm(LK);
     __shared__ int2 s_queue[4][QCAP];
+    __shared__ double s_T[4][3][NIMG_J];
+    __shared__ float s_C[4][3][NIMG_J];
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-    const int ib = blockIdx.x * 4 + w;
+    int ib = blockIdx.x * 4 + w;
+    if (p.shard_n > 1) ib = ib * p.shard_n + p.shard_rank;
     if (ib >= nbra) return;
+    const KetListJ &KJ = p.KJ;
+    const Lattice &lat = p.lat;
     const int u = __ldg(bra_idx + ib);
     const double Pix = p.U.Px[u], Piy = p.U.Py[u], Piz = p.U.Pz[u];
     const double pi_ = p.U.p[u], coefi = p.U.coef[u];
-    const double ipi = p.U.ip[u];
-    const double thr = p.U.lb[u] + *p.lnPmax - p.ln_tau;
+    const float ipi = (float)p.U.ip[u];
+    const float M = SCREEN_MARGIN;
+    const float ln_tau = (float)p.ln_tau;
+    const float lbi = (float)p.U.lb[u];
+    const float thr = lbi + (float)*p.lnPmax - ln_tau;          // level A: global max |P'|
+    const float thrx = lbi - ln_tau;                              // level B refinement: + per-ket block max
+    const float iw2 = (float)lat.iomega2;
+    const float rcut2f = p.rcut2 < 1e30 ? (float)p.rcut2 * 1.00001f : 3.0e38f;
     double Jt[NT];
 #pragma unroll
     for (int t = 0; t < NT; ++t) Jt[t] = 0.0;
-    int qn = 0;
-    unsigned ncand = 0, nq = 0;
     int2 *queue = s_queue[w];
-    const Lattice &lat = p.lat;
-    const double *__restrict__ tab = p.boys;
+    double *sT = &s_T[w][0][0];
+    float *sC = &s_C[w][0][0];
+    const unsigned ltmask = (1u << lane) - 1u;
+    unsigned ncand = 0;
+    unsigned long long nquart = 0;
+    int head = 0, qn = 0;
 
-    auto eval = [&](int j, int timg) {
-        double Tx, Ty, Tz;
-        unpack_img(timg, lat, Tx, Ty, Tz);
-        const double X = __ldg(p.KJ.Qx + j) + Tx - Pix, Y = __ldg(p.KJ.Qy + j) + Ty - Piy,
-                     Z = __ldg(p.KJ.Qz + j) + Tz - Piz;
-        const double q = __ldg(p.KJ.q + j);
-        const double r2 = X * X + Y * Y + Z * Z;
-        const double s = rsqrt(pi_ + q);
-        const double alpha = pi_ * q * s * s;
-        const double th = lat.omega * rsqrt(alpha + lat.omega2);
-        const double alpha_w = alpha * th * th;
-        const double pref = coefi * __ldg(p.KJ.coef + j) * s;
-        double Rm[L + 1];
-        boys_merged<L>(tab, r2, alpha, alpha_w, th, pref, Rm);
-        double R[nherm(L)];
-        hermite_R<L>(R, Rm, X, Y, Z);
-        double D[NS];
-#pragma unroll
-        for (int sI = 0; sI < NS; ++sI) D[sI] = __ldg(p.Dt + (size_t)sI * p.KJ.dstride + j);
-#pragma unroll
-        for (int tx = 0; tx <= LB; ++tx)
-#pragma unroll
-            for (int ty = 0; ty <= LB - tx; ++ty)
-#pragma unroll
-                for (int tz = 0; tz <= LB - tx - ty; ++tz) {
-                    double acc = Jt[hidx(tx, ty, tz)];
-#pragma unroll
-                    for (int sx = 0; sx <= LK; ++sx)
-#pragma unroll
-                        for (int sy = 0; sy <= LK - sx; ++sy)
-#pragma unroll
-                            for (int sz = 0; sz <= LK - sx - sy; ++sz)
-                                acc = fma(R[hidx(tx + sx, ty + sy, tz + sz)], D[hidx(sx, sy, sz)], acc);
-                    Jt[hidx(tx, ty, tz)] = acc;
-                }
-    };
-
-    for (int g = 0; g < p.KJ.ngroup; ++g) {
-        const int gi = g * 5 + LK;
-        const int k0 = __ldg(p.KJ.off + gi), k1 = __ldg(p.KJ.off + gi + 1);
-        if (k1 <= k0) continue;
-        scan_group(lat, Pix, Piy, Piz, ipi, thr, __ldg(p.KJ.gx + g), __ldg(p.KJ.gy + g), __ldg(p.KJ.gz + g),
-                   __ldg(p.KJ.ext + gi), __ldg(p.KJ.iqmax + gi), k0, k1, p.KJ.Qx, p.KJ.Qy, p.KJ.Qz, p.KJ.iq,
-                   p.KJ.lb, p.rcut2, queue, qn, lane, ncand, nq, eval);
+    // images of the whole ket set within reach of this bra: sphere around P - g0 (g0 = cell centre; every atom
+    // lies within KJ.rc of it), radius = reach of the strongest ket of order LK + its extent + rc
+    const float budget_all = thr + KJ.lbmax[LK] + M;
+    ImageBox box;
+    box.n = 0;
+    double Rall = 0.0;
+    const double c0x = Pix - KJ.g0[0], c0y = Piy - KJ.g0[1], c0z = Piz - KJ.g0[2];
+    if (budget_all > 0.f) {
+        Rall = sqrt((double)budget_all * (double)(ipi + KJ.iqmaxall[LK] + iw2)) + KJ.extmax[LK] + KJ.rc + 1e-3;
+        box.set(lat, c0x, c0y, c0z, Rall);
     }
-    if (qn > 0) {                                   // flush: partial warp
-        if (lane < qn) {
-            const int2 e = queue[lane];
-            eval(e.x, e.y);
+    const int natom = KJ.ngroup;
+    for (int ibox = 0; ibox < box.n;) {
+        // ---- image list chunk of this warp ----
+        int nimg = 0;
+        __syncwarp();
+        while (ibox < box.n && nimg <= NIMG_J - 32) {
+            const int im = ibox + lane;
+            bool ok = false;
+            double Tx = 0, Ty = 0, Tz = 0;
+            if (im < box.n) {
+                int n0, n1, n2;
+                box.decode(im, n0, n1, n2);
+                lattice_T(lat, n0, n1, n2, Tx, Ty, Tz);
+                const double ex = c0x - Tx, ey = c0y - Ty, ez = c0z - Tz;
+                ok = ex * ex + ey * ey + ez * ez <= Rall * Rall;
+            }
+            const unsigned m = __ballot_sync(0xffffffffu, ok);
+            if (ok) {
+                const int pos = nimg + __popc(m & ltmask);
+                sT[pos] = Tx; sT[NIMG_J + pos] = Ty; sT[2 * NIMG_J + pos] = Tz;
+                sC[pos] = (float)(c0x - Tx); sC[NIMG_J + pos] = (float)(c0y - Ty); sC[2 * NIMG_J + pos] = (float)(c0z - Tz);
+            }
+            nimg += __popc(m);
+            ibox += 32;
+        }
+        __syncwarp();
+        const int nitems = natom * nimg;
+        int ebase = 0;
+        unsigned imask = 0;
+        bool have = false, items_done = false;
+        // per-lane item, current item
+        int it_cnt = 0, it_k0 = 0, it_t = 0;
+        float it_Dx = 0.f, it_Dy = 0.f, it_Dz = 0.f;
+        int c_cnt = 0, c_k0 = 0, c_t = 0, jpos = 0;
+        float c_Dx = 0.f, c_Dy = 0.f, c_Dz = 0.f;
+        for (;;) {
+            while (qn < 32) {
+                if (!have) {
+                    if (imask == 0) {
+                        if (ebase >= nitems) { items_done = true; break; }
+                        const int e = ebase + lane;
+                        ebase += 32;
+                        it_cnt = 0;
+                        if (e < nitems) {
+                            const int a = e / nimg, t = e - a * nimg;
+                            const int gi = a * 5 + LK;
+                            const int2 go = __ldg(KJ.goff + gi);                   // (first ket, count)
+                            if (go.y > 0) {
+                                const float4 gr = __ldg(KJ.grec + gi);             // (ext, iqmax, lbmax, -)
+                                const float4 ga = __ldg(KJ.g4 + a);                // atom position - g0
+                                const float Dx = sC[t] - ga.x, Dy = sC[NIMG_J + t] - ga.y, Dz = sC[2 * NIMG_J + t] - ga.z;
+                                const float dist = sqrtf(Dx * Dx + Dy * Dy + Dz * Dz);
+                                const float dlb = fmaxf(dist * (1.f - 4e-6f) - gr.x - 1e-4f, 0.f);
+                                const float need = __fdividef(dlb * dlb, ipi + gr.y + iw2) - thr - 2.f * M;
+                                if (need < gr.z) {                                 // the strongest ket could survive
+                                    it_cnt = count_above_sorted(KJ.q4 + go.x, go.y, need);   // kets sorted by bound
+                                    it_k0 = go.x; it_t = t; it_Dx = Dx; it_Dy = Dy; it_Dz = Dz;
+                                }
+                            }
+                        }
+                        imask = __ballot_sync(0xffffffffu, it_cnt > 0);
+                        continue;
+                    }
+                    const int src = __ffs(imask) - 1;
+                    imask &= imask - 1;
+                    c_cnt = __shfl_sync(0xffffffffu, it_cnt, src);
+                    c_k0 = __shfl_sync(0xffffffffu, it_k0, src);
+                    c_t = __shfl_sync(0xffffffffu, it_t, src);
+                    c_Dx = __shfl_sync(0xffffffffu, it_Dx, src);
+                    c_Dy = __shfl_sync(0xffffffffu, it_Dy, src);
+                    c_Dz = __shfl_sync(0xffffffffu, it_Dz, src);
+                    jpos = 0;
+                    have = true;
+                }
+                if (jpos >= c_cnt) { have = false; continue; }
+                const int jj = jpos + lane;
+                jpos += 32;
+                bool pass = false;
+                if (jj < c_cnt) {
+                    const int j = c_k0 + jj;
+                    const float4 k4 = __ldg(KJ.q4 + j);                           // (Q - atom).xyz, lb
+                    const float iq = __ldg(KJ.iqf + j);
+                    const float ex = k4.x - c_Dx, ey = k4.y - c_Dy, ez = k4.z - c_Dz;   // Q + T - P
+                    const float r2 = ex * ex + ey * ey + ez * ez;
+                    const float isum = ipi + iq + iw2;
+                    pass = (thr + k4.w + M) * isum > r2 && r2 <= rcut2f;
+                    if (pass) pass = (thrx + k4.w + __ldg(p.kjP + j) + M) * isum > r2;   // per-block max |P'| (L819)
+                    ++ncand;
+                }
+                const unsigned m = __ballot_sync(0xffffffffu, pass);
+                if (pass) queue[(head + qn + __popc(m & ltmask)) & (QCAP - 1)] = make_int2(c_k0 + jj, c_t);
+                qn += __popc(m);
+                __syncwarp();
+            }
+            if (!(qn >= 32 || (items_done && qn > 0))) break;
+            // ---- evaluation: one primitive quartet-image per lane ----
+            const int take = qn < 32 ? qn : 32;
+            if (lane < take) {
+                const int2 e = queue[(head + lane) & (QCAP - 1)];
+                const int j = e.x, t = e.y;
+                const double X = __ldg(KJ.Qx + j) + sT[t] - Pix, Y = __ldg(KJ.Qy + j) + sT[NIMG_J + t] - Piy,
+                             Z = __ldg(KJ.Qz + j) + sT[2 * NIMG_J + t] - Piz;
+                const double q = __ldg(KJ.q + j);
+                const double r2 = X * X + Y * Y + Z * Z;
+                const double s = rsqrt(pi_ + q);
+                const double alpha = pi_ * q * s * s;
+                const double th = lat.omega * rsqrt(alpha + lat.omega2);
+                const double alpha_w = alpha * th * th;
+                const double pref = r2 <= p.rcut2 ? coefi * __ldg(KJ.coef + j) * s : 0.0;
+                double Rm[L + 1];
+                boys_merged<L, double>(p.boys, r2, alpha, alpha_w, th, pref, Rm);
+                double R[nherm(L)];
+                hermite_R<L>(R, Rm, X, Y, Z);
+                double D[NS];
+#pragma unroll
+                for (int sI = 0; sI < NS; ++sI) D[sI] = __ldg(p.Dt + (size_t)sI * KJ.dstride + j);
+#pragma unroll
+                for (int tx = 0; tx <= LB; ++tx)
+#pragma unroll
+                    for (int ty = 0; ty <= LB - tx; ++ty)
+#pragma unroll
+                        for (int tz = 0; tz <= LB - tx - ty; ++tz) {
+                            double acc = Jt[hidx(tx, ty, tz)];
+#pragma unroll
+                            for (int sx = 0; sx <= LK; ++sx)
+#pragma unroll
+                                for (int sy = 0; sy <= LK - sx; ++sy)
+#pragma unroll
+                                    for (int sz = 0; sz <= LK - sx - sy; ++sz)
+                                        acc = fma(R[hidx(tx + sx, ty + sy, tz + sz)], D[hidx(sx, sy, sz)], acc);
+                            Jt[hidx(tx, ty, tz)] = acc;
+                        }
+            }
+            head = (head + take) & (QCAP - 1);
+            qn -= take;
+            nquart += take;
+            __syncwarp();
         }
     }
     // warp reduction (fixed order => deterministic)
@@ -228,12 +302,12 @@ __global__ void __launch_bounds__(128) sr_j_kernel(SRParams p, const int *__rest
         for (int t = 0; t < NT; ++t) p.Jt[(size_t)t * p.U.n + u] += Jt[t];
     }
     // statistics (once per warp, not on the data path)
-    unsigned long long c = ncand, e32 = (unsigned long long)nq * 32ull;
+    unsigned long long c = ncand;
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) c += __shfl_xor_sync(0xffffffffu, c, o);
     if (lane == 0) {
         atomicAdd(p.counters + CNT_CAND_J + LB * 5 + LK, c);
-        atomicAdd(p.counters + CNT_Q_J + LB * 5 + LK, e32 + (unsigned long long)qn);
+        atomicAdd(p.counters + CNT_Q_J + LB * 5 + LK, nquart);
     }
 }
 
@@ -250,8 +324,10 @@ __host__ __device__ constexpr int bra_terms()
     return n;
 }
 
-// launchers (defined in the instantiation units)
+// launchers (defined in the instantiation units); `mixed` selects the fp64+fp32 K kernels
 void launch_sr_j(int LB, int LK, const SRParams &p, const int *bra_idx, int nbra, cudaStream_t st);
-void launch_sr_k(int la, int lb, int lc, int ld, const SRParams &p, const int2 *blocks, int nblocks, cudaStream_t st);
+void launch_sr_k(int la, int lb, int lc, int ld, bool mixed, const SRParams &p, const int2 *blocks, int nblocks, cudaStream_t st);
+// opt in to the dynamic shared memory of every K class on the current device (once per handle)
+void sr_k_set_attributes();
 
 }  // namespace pbcjk

@@ -1,15 +1,23 @@
 // Real-space K kernels (eq 74 L558 with eq 56/69): class (LA LB | LC LD), bra = (mu: LA, lambda: LB),
-// ket = (nu: LD, sigma: LC).  One CTA owns the output block (mu, nu); warps take the bra primitive
-// pair-images of mu round-robin; lanes the ket primitive pair-images of nu and the lattice image R1.
+// ket = (nu: LD, sigma: LC).  One CTA owns the output block (mu, nu):
 //   K[mu_a, nu_d] += sum P'[lambda_b, sigma_c] (mu_a lambda_b | sigma_c nu_d)
 //
-// Phase 1 (scan) is the same screen as the J-engine's scan_group (eq 67, bounding box eq 99-103),
-// written as a resumable iterator so that the quartet evaluator -- straight-line code generated per
-// class by gen_sr_k.py -- is expanded at exactly one call site.  Survivors wait in a per-warp ring that
-// spans several bras (each keeps its E row and centre in a shared-memory slot), so the evaluator runs
-// with 32 active lanes except for the last call of a warp.  The Hermite integrals of classes with
-// L > 4 live in shared memory (one column per thread); the E products of both pairs come from the
-// tables built at create (PairListK::etab), so no E recursion runs per quartet.
+// Screen (see pbcjk_sr.cuh): the CTA lists the lattice images R1 that can couple the bra group (mu, all lambda of
+// class LB) with the ket group (nu, all sigma of class LC) once (eq 99-103: bounding box, then sphere filter); an
+// ITEM is a (bra primitive pair-image, image) pair; the warps take the items 32 at a time, one per lane (level A:
+// distance to the ket group, the bound a ket needs there, number of kets above it by binary search in the list sorted
+// by bound), then test the kets of every live item in fp32 (level B: eq 67 with the row maximum of |P'|, then with
+// the maximum over the shell block (lambda, sigma), L819).  Survivors wait in a per-warp ring as (bra, ket, image);
+// whenever 32 are queued each lane evaluates one primitive quartet-image with the straight-line evaluator generated
+// per class by gen_sr_k.py.  The Hermite integrals of classes with L > 4 live in shared memory (one column per
+// thread); the E products of both pairs come from the tables built at create (PairListK::etab), so no E recursion
+// runs per quartet.
+//
+// MIXED (PAPER 3.5 L817-821): a second ring takes the survivors whose ln(bound_bra bound_ket max|P block|) is below
+// ln(mixed_switch); they run the same evaluator instantiated for float (fp32 tables, fp32 density), accumulated
+// into the fp64 block sums.  The bound used for the switch leaves out the exp(-alpha_w r^2) factor of eq 67 on
+// purpose: the erfc-attenuated integral is a difference of two Boys terms, and fp32 rounding acts on the terms, not
+// on their difference.
 #pragma once
 #include "pbcjk_sr.cuh"
 
@@ -17,225 +25,311 @@ namespace pbcjk {
 
 template <int LA, int LB, int LC, int LD> struct KEval;      // specialisations: build/gen/k_eval_*.cuh
 
+__device__ __forceinline__ double ldg_volatile(const double *p)
+{
+    double v;
+    asm volatile("ld.global.nc.f64 %0, [%1];" : "=d"(v) : "l"(p));
+    return v;
+}
+__device__ __forceinline__ float ldg_volatile(const float *p)
+{
+    float v;
+    asm volatile("ld.global.nc.f32 %0, [%1];" : "=f"(v) : "l"(p));
+    return v;
+}
+
 // CTA size: 128 threads in every class.  The warps of a CTA enter the evaluator in lockstep at L >= 5 (see LOCKSTEP
 // below), so four warps share the instruction fetches; the R column of a thread takes 8*nherm(L) bytes of shared
-// memory (1320 B at L = 8: one CTA per SM).  Measured on water64 / si64: 64-thread CTAs at L >= 7 are 3 % slower,
-// 256-thread CTAs at L = 5 are 4-6 % slower, lockstep at L = 3, 4 is 10 % slower.
+// memory (1320 B at L = 8: one CTA per SM).
 __host__ __device__ constexpr int k_nthreads(int) { return 128; }
-
-// bra slots per warp: a queued quartet refers to its bra by slot, so the queue carries survivors across bras
-// and the evaluator runs with (nearly) all 32 lanes; the slot stride is odd so that lanes reading the E tables
-// of different slots hit different banks.
-__host__ __device__ constexpr int k_nslot(int nterm, int) { return nterm > 150 ? 4 : 8; }
-__host__ __device__ constexpr int k_slot_stride(int nterm) { return (nterm + 6) | 1; }   // E row + 6 scalars, odd
+#define K_MIXED_LMAX 4                                        // highest class order with a mixed-precision kernel
 constexpr int KQ = 64;                                       // ring capacity per warp (power of two)
+constexpr int NIMG_K = 128;                                  // lattice images per CTA-level list chunk
 
-template <int LA, int LB, int LC, int LD>
+
+template <int LA, int LB, int LC, int LD, bool MIXED>
 constexpr size_t k_smem_bytes()
 {
     constexpr int L = LA + LB + LC + LD, NT = k_nthreads(L), NW = NT / 32;
-    constexpr int NTERM = bra_terms<LA, LB>();
-    size_t d = (L > 4 ? (size_t)nherm(L) * NT : 0) + (size_t)NW * k_nslot(NTERM, L) * k_slot_stride(NTERM) +
-               (size_t)NW * ncart(LA) * ncart(LD);
-    return d * sizeof(double) + (size_t)NW * KQ * (sizeof(int2) + sizeof(int));
+    size_t d = (L > 4 ? (size_t)nherm(L) * NT : 0) + (size_t)NW * ncart(LA) * ncart(LD) + 3 * NIMG_K;
+    return d * sizeof(double) + 3 * NIMG_K * sizeof(float) + (size_t)NW * KQ * sizeof(int2) * (MIXED ? 2 : 1);
 }
 
 // light classes: at most 128 registers (L <= 3: 4 CTAs, 16 warps per SM) or 168 (L = 4: 3 CTAs); the few spilled
-// doubles (<= 300 B per thread) cost less than the lost occupancy
+// doubles cost less than the lost occupancy
 __host__ __device__ constexpr int k_minblocks(int L) { return L <= 3 ? 4 : (L == 4 ? 3 : 1); }
 
-template <int LA, int LB, int LC, int LD>
+// CTA-wide: number of leading entries (sorted by descending q4[].w) above `bound`
+__device__ __forceinline__ int count_above_cta(const float4 *__restrict__ q4, int n, float bound)
+{
+    int tot = 0;
+    for (int base = 0; base < n; base += blockDim.x) {
+        const int idx = base + threadIdx.x;
+        const int c = __syncthreads_count(idx < n && __ldg(&q4[idx].w) > bound);
+        tot += c;
+        if (c < (int)blockDim.x) break;
+    }
+    return tot;
+}
+
+template <int LA, int LB, int LC, int LD, bool MIXED>
 __global__ void __launch_bounds__(k_nthreads(LA + LB + LC + LD), k_minblocks(LA + LB + LC + LD))
 sr_k_kernel(SRParams p, const int2 *__restrict__ blocks, int nblocks)
 {
     constexpr int L = LA + LB + LC + LD;
     constexpr int NT = k_nthreads(L), NW = NT / 32;
     constexpr int NA = ncart(LA), ND = ncart(LD);
-    constexpr int NTERM = bra_terms<LA, LB>();
-    constexpr int NSLOT = k_nslot(NTERM, L), SSTR = k_slot_stride(NTERM);
     constexpr bool RSMEM = L > 4;
     constexpr bool LOCKSTEP = L >= 5;
     using Ev = KEval<LA, LB, LC, LD>;
-    static_assert(Ev::NBRA == NTERM, "generator and kernel disagree on the bra table");
+    static_assert(Ev::NBRA == bra_terms<LA, LB>(), "generator and kernel disagree on the bra table");
     extern __shared__ __align__(16) double smem[];
-    double *Rs = smem + threadIdx.x;                                  // [nherm(L)][NT] when RSMEM
-    double *sB = smem + (RSMEM ? nherm(L) * NT : 0);                  // [NW][NSLOT][SSTR]: E row, Px,Py,Pz,p,coef,aoB
-    double *s_red = sB + NW * NSLOT * SSTR;                           // [NW][NA*ND]
-    int2 *queue = reinterpret_cast<int2 *>(s_red + NW * NA * ND);     // [NW][KQ] (ket, packed image)
-    int *qbra = reinterpret_cast<int *>(queue + NW * KQ);             // [NW][KQ] running number of the bra
+    // R columns when RSMEM: [warp][nherm(L)][32], one column per thread inside the warp's own slice -- the float columns of
+    // a warp's fp32 pass (MIXED) reuse that slice, so warps evaluating in different precisions never touch each other
+    double *Rs = smem + (size_t)(threadIdx.x >> 5) * nherm(L) * 32 + (threadIdx.x & 31);
+    double *s_red = smem + (RSMEM ? nherm(L) * NT : 0);               // [NW][NA*ND]
+    double *sT = s_red + NW * NA * ND;                                // [3][NIMG_K] lattice vectors of the image list
+    float *sC = reinterpret_cast<float *>(sT + 3 * NIMG_K);           // [3][NIMG_K] centre(mu) - centre(nu) - T
+    int2 *queue = reinterpret_cast<int2 *>(sC + 3 * NIMG_K);          // [NW][KQ] (bra | ket << 16, image)
+    int2 *queue32 = queue + NW * KQ;                                  // [NW][KQ] fp32 ring (MIXED)
+    __shared__ int s_ctl[2];
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-    sB += w * NSLOT * SSTR;
     queue += w * KQ;
-    qbra += w * KQ;
-    const int2 blk = blocks[blockIdx.x];
+    queue32 += w * KQ;
+    const PairListK &K = p.K;
+    const int bidx = p.shard_n > 1 ? blockIdx.x * p.shard_n + p.shard_rank : blockIdx.x;
+    if (bidx >= nblocks) return;
+    const int2 blk = blocks[bidx];
     const int mu = blk.x, nu = blk.y;
-    const int b0 = __ldg(p.K.off + mu * 3 + LB), b1 = __ldg(p.K.off + mu * 3 + LB + 1);
-    const int k0 = __ldg(p.K.off + nu * 3 + LC), k1 = __ldg(p.K.off + nu * 3 + LC + 1);
+    const int b0 = __ldg(K.off + mu * 3 + LB), b1 = __ldg(K.off + mu * 3 + LB + 1);
+    const int k0 = __ldg(K.off + nu * 3 + LC), k1 = __ldg(K.off + nu * 3 + LC + 1);
     if (b1 <= b0 || k1 <= k0) return;
     const Lattice &lat = p.lat;
-    const double *__restrict__ tab = p.boys;
-    const int N = p.sh.nbf;
-    const double gx = __ldg(p.sh.cx + nu), gy = __ldg(p.sh.cy + nu), gz = __ldg(p.sh.cz + nu);
-    const double kext = __ldg(p.K.ext + nu * 3 + LC), kiqmax = __ldg(p.K.ipmax + nu * 3 + LC);
-    const double lbmax_ket = __ldg(p.K.lb + k0);
-    const double thr0 = *p.lnPmax - p.ln_tau;
-    const double *__restrict__ kQx = p.K.Px, *__restrict__ kQy = p.K.Py, *__restrict__ kQz = p.K.Pz;
-    const double *__restrict__ kiq = p.K.ip, *__restrict__ klb = p.K.lb;
+    const int N = p.sh.nbf, ns = p.sh.nshell;
+    const float M = SCREEN_MARGIN;
+    const float ln_tau = (float)p.ln_tau;
+    const float lnPmax = (float)*p.lnPmax;
+    const float iw2 = (float)lat.iomega2;
+    const float rcut2f = p.rcut2 < 1e30 ? (float)p.rcut2 * 1.00001f : 3.0e38f;
+    const float lbmax_bra = __ldg(&K.q4[b0].w), lbmax_ket = __ldg(&K.q4[k0].w);
+    const float budget_blk = lbmax_bra + lbmax_ket + lnPmax - ln_tau + M;
+    if (budget_blk <= 0.f) return;
+    // entries that can survive at all (lists sorted by bound)
+    const int nb_eff = count_above_cta(K.q4 + b0, b1 - b0, -(lbmax_ket + lnPmax - ln_tau + M));
+    const int nk_eff = count_above_cta(K.q4 + k0, k1 - k0, -(lbmax_bra + lnPmax - ln_tau + M));
+    const float kext = (float)__ldg(K.ext + nu * 3 + LC), kiqmax = (float)__ldg(K.ipmax + nu * 3 + LC);
+    const float4 *__restrict__ kq4 = K.q4 + k0;
+    const float *__restrict__ kipf = K.ipf + k0;
+    const int *__restrict__ kshB = K.shB + k0;
     const unsigned ltmask = (1u << lane) - 1u;
+
+    // lattice images within reach of the two groups: sphere around centre(mu) - centre(nu)
+    const double cx = __ldg(p.sh.cx + mu) - __ldg(p.sh.cx + nu), cy = __ldg(p.sh.cy + mu) - __ldg(p.sh.cy + nu),
+                 cz = __ldg(p.sh.cz + mu) - __ldg(p.sh.cz + nu);
+    const double Rblk = sqrt((double)budget_blk * ((double)__ldg(K.ipmax + mu * 3 + LB) + kiqmax + iw2)) + kext +
+                        __ldg(K.ext + mu * 3 + LB) + 1e-3;
+    ImageBox box;
+    box.set(lat, cx, cy, cz, Rblk);
 
     double Kacc[NA * ND];
 #pragma unroll
     for (int i = 0; i < NA * ND; ++i) Kacc[i] = 0.0;
     unsigned ncand = 0;
-    unsigned long long nquart = 0;
+    unsigned long long nquart = 0, nquart32 = 0;
+    int head = 0, qn = 0, head32 = 0, qn32 = 0;
 
-    // scan state of the warp (all warp-uniform except need_l, timg_l)
-    int i = b0 + w;                       // next / current bra primitive pair-image
-    int bcnt = 0;                         // bras started so far; the current one is number bcnt - 1
-    bool bra_active = false, have = false;
-    int head = 0, qn = 0;                 // ring of survivors
-    int base = 0, nimg = 0, j0 = k0, timg = 0, timg_l = 0;
-    int lo0 = 0, lo1 = 0, lo2 = 0, d2 = 1, d12 = 1;
-    unsigned imask = 0;
-    double thr = 0.0, ipi = 0.0, Pix = 0.0, Piy = 0.0, Piz = 0.0, cx = 0.0, cy = 0.0, cz = 0.0;
-    double inv_isum_max = 0.0, rho2 = 0.0, need = 0.0, need_l = 0.0, ox = 0.0, oy = 0.0, oz = 0.0;
-
-    for (;;) {
-        // ---- phase 1: screen (bra, ket, image) candidates until 32 survivors are queued ----
-        while (qn < 32) {
-            if (!bra_active) {
-                if (i >= b1) break;                                   // no bra left
-                thr = __ldg(p.K.lb + i) + thr0;
-                const double budget = thr + lbmax_ket;
-                if (budget <= 0.0) { i = b1; break; }                 // bras sorted: the rest is weaker
-                // the slot this bra takes must not be referenced by a queued survivor any more
-                if (qn > 0 && bcnt - qbra[head] >= NSLOT) break;      // evaluate what is queued first
-                double *slot = sB + (bcnt % NSLOT) * SSTR;
-                Pix = __ldg(p.K.Px + i); Piy = __ldg(p.K.Py + i); Piz = __ldg(p.K.Pz + i);
-                ipi = __ldg(p.K.ip + i);
-                {
-                    const double *__restrict__ src = p.K.etab + __ldg(p.K.eoff + i);
-                    __syncwarp();
-                    for (int n = lane; n < NTERM; n += 32) slot[n] = __ldg(src + n);
-                    if (lane == 0) {
-                        slot[NTERM] = Pix; slot[NTERM + 1] = Piy; slot[NTERM + 2] = Piz;
-                        slot[NTERM + 3] = __ldg(p.K.p + i); slot[NTERM + 4] = __ldg(p.K.coef + i);
-                        slot[NTERM + 5] = (double)__ldg(p.K.aoB + i);
-                    }
-                    __syncwarp();
+    for (int ibox = 0; ibox < box.n;) {
+        // ---- CTA-level image list chunk, filled by warp 0 in box order (deterministic) ----
+        __syncthreads();
+        if (w == 0) {
+            int n = 0, ib = ibox;
+            while (ib < box.n && n <= NIMG_K - 32) {
+                const int im = ib + lane;
+                bool ok = false;
+                double Tx = 0, Ty = 0, Tz = 0;
+                if (im < box.n) {
+                    int n0, n1, n2;
+                    box.decode(im, n0, n1, n2);
+                    lattice_T(lat, n0, n1, n2, Tx, Ty, Tz);
+                    const double ex = cx - Tx, ey = cy - Ty, ez = cz - Tz;
+                    ok = ex * ex + ey * ey + ez * ez <= Rblk * Rblk;
                 }
-                // bounding box of the lattice images within reach of the ket group (eq 99-103)
-                const double isum_max = ipi + kiqmax + lat.iomega2;
-                const double rho = sqrt(budget * isum_max) + kext;
-                cx = Pix - gx; cy = Piy - gy; cz = Piz - gz;
-                const double f0 = lat.binv[0] * cx + lat.binv[1] * cy + lat.binv[2] * cz;
-                const double f1 = lat.binv[3] * cx + lat.binv[4] * cy + lat.binv[5] * cz;
-                const double f2 = lat.binv[6] * cx + lat.binv[7] * cy + lat.binv[8] * cz;
-                lo0 = (int)ceil(f0 - rho * lat.bnorm[0]);
-                lo1 = (int)ceil(f1 - rho * lat.bnorm[1]);
-                lo2 = (int)ceil(f2 - rho * lat.bnorm[2]);
-                const int hi0 = (int)floor(f0 + rho * lat.bnorm[0]), hi1 = (int)floor(f1 + rho * lat.bnorm[1]);
-                const int hi2 = (int)floor(f2 + rho * lat.bnorm[2]);
-                const int d1 = hi1 - lo1 + 1;
-                d2 = hi2 - lo2 + 1;
-                d12 = d1 * d2;
-                nimg = (hi0 >= lo0 && d1 > 0 && d2 > 0) ? (hi0 - lo0 + 1) * d12 : 0;
-                inv_isum_max = 1.0 / isum_max;
-                rho2 = rho * rho;
-                base = 0; imask = 0; have = false;
-                bra_active = true;
-                ++bcnt;
-            }
-            if (!have) {
-                if (imask == 0) {
-                    if (base >= nimg) { bra_active = false; i += NW; continue; }     // this bra is done
-                    // 32 images of the box at a time, one per lane: sphere filter and the bound each image
-                    // needs from a ket (eq 67 at the closest approach of the ket group)
-                    const int im = base + lane;
-                    base += 32;
-                    bool ok = false;
-                    if (im < nimg) {
-                        const int n0 = lo0 + im / d12, r = im % d12;
-                        const int n1 = lo1 + r / d2, n2 = lo2 + r % d2;
-                        const double Tx = n0 * lat.a[0] + n1 * lat.a[3] + n2 * lat.a[6];
-                        const double Ty = n0 * lat.a[1] + n1 * lat.a[4] + n2 * lat.a[7];
-                        const double Tz = n0 * lat.a[2] + n1 * lat.a[5] + n2 * lat.a[8];
-                        const double ex = Tx - cx, ey = Ty - cy, ez = Tz - cz;
-                        const double dist2 = ex * ex + ey * ey + ez * ez;
-                        ok = dist2 <= rho2;
-                        double dlb = sqrt(dist2) - kext;        // lower bound of |Q + T - P|
-                        dlb = dlb > 0.0 ? dlb : 0.0;
-                        need_l = dlb * dlb * inv_isum_max - thr;   // a ket survives only if lb_ket > need
-                        timg_l = pack_img(n0, n1, n2);
-                    }
-                    imask = __ballot_sync(0xffffffffu, ok);
-                    continue;
+                const unsigned m = __ballot_sync(0xffffffffu, ok);
+                if (ok) {
+                    const int pos = n + __popc(m & ltmask);
+                    sT[pos] = Tx; sT[NIMG_K + pos] = Ty; sT[2 * NIMG_K + pos] = Tz;
+                    sC[pos] = (float)(cx - Tx); sC[NIMG_K + pos] = (float)(cy - Ty); sC[2 * NIMG_K + pos] = (float)(cz - Tz);
                 }
-                const int src = __ffs(imask) - 1;
-                imask &= imask - 1;
-                need = __shfl_sync(0xffffffffu, need_l, src);
-                timg = __shfl_sync(0xffffffffu, timg_l, src);
-                double Tx, Ty, Tz;
-                unpack_img(timg, lat, Tx, Ty, Tz);
-                ox = Tx - Pix; oy = Ty - Piy; oz = Tz - Piz;
-                j0 = k0;
-                have = true;
+                n += __popc(m);
+                ib += 32;
             }
-            if (j0 >= k1 || __ldg(klb + j0) <= need) { have = false; continue; }   // sorted by lb
-            const int j = j0 + lane;
-            bool pass = false;
-            if (j < k1) {
-                const double dx = __ldg(kQx + j) + ox, dy = __ldg(kQy + j) + oy, dz = __ldg(kQz + j) + oz;
-                const double r2 = dx * dx + dy * dy + dz * dz;
-                const double isum = ipi + __ldg(kiq + j) + lat.iomega2;
-                pass = (thr + __ldg(klb + j)) * isum > r2 && r2 <= p.rcut2;
-                ++ncand;
-            }
-            const unsigned m = __ballot_sync(0xffffffffu, pass);
-            if (pass) {
-                const int pos = (head + qn + __popc(m & ltmask)) & (KQ - 1);
-                queue[pos] = make_int2(j, timg);
-                qbra[pos] = bcnt - 1;
-            }
-            qn += __popc(m);
-            j0 += 32;
-            __syncwarp();
+            if (lane == 0) { s_ctl[0] = n; s_ctl[1] = ib; }
         }
-        if (LOCKSTEP) {
-            // the evaluators of the high classes are 10-60 thousand instructions of straight-line code, far more than
-            // the instruction caches hold (ncu: 45 % of the stall samples of (dp|dp) were "no instruction"); the warps
-            // of a CTA therefore enter the evaluator together and share the fetched lines.  Every warp passes this
-            // barrier once per round until no warp has anything queued.
-            if (!__syncthreads_or(qn > 0)) break;
-            if (qn == 0) continue;
-        } else if (qn == 0) break;                                    // nothing queued and no bra left
-        // ---- phase 2: one primitive quartet-image per lane, oldest survivors first ----
-        const int take = qn < 32 ? qn : 32;
-        if (lane < take) {
-            const int pos = (head + lane) & (KQ - 1);
-            const int2 e = queue[pos];
-            const double *__restrict__ slot = sB + (qbra[pos] % NSLOT) * SSTR;
-            const int j = e.x;
-            double Tx, Ty, Tz;
-            unpack_img(e.y, lat, Tx, Ty, Tz);
-            const double X = __ldg(kQx + j) + Tx - slot[NTERM], Y = __ldg(kQy + j) + Ty - slot[NTERM + 1],
-                         Z = __ldg(kQz + j) + Tz - slot[NTERM + 2];
-            const double pb = slot[NTERM + 3], q = __ldg(p.K.p + j);
-            const double r2 = X * X + Y * Y + Z * Z;
-            const double s = rsqrt(pb + q);
-            const double alpha = pb * q * s * s;
-            const double th = lat.omega * rsqrt(alpha + lat.omega2);
-            const double alpha_w = alpha * th * th;
-            const double pref = slot[NTERM + 4] * __ldg(p.K.coef + j) * s;
-            const double *__restrict__ Pb = p.Pp + (size_t)(int)slot[NTERM + 5] * p.ldP + __ldg(p.K.aoB + j);
-            double Rm[L + 1];
-            boys_merged<L>(tab, r2, alpha, alpha_w, th, pref, Rm);
-            Ev::template run<NT>(slot, p.K.etab + __ldg(p.K.eoff + j), Pb, p.ldP, Rm, X, Y, Z, Rs, Kacc);
+        __syncthreads();
+        const int nimg = s_ctl[0];
+        ibox = s_ctl[1];
+        const int nitems = nb_eff * nimg;
+        int ebase = w * 32;
+        unsigned imask = 0;
+        bool have = false, items_done = false;
+        // per-lane item (level A result) and the item being scanned (warp-uniform)
+        int it_cnt = 0, it_ibt = 0, c_ibt = 0, c_cnt = 0, jpos = 0;  // it_ibt: bra | image << 16
+        float it_Dx = 0.f, it_Dy = 0.f, it_Dz = 0.f, it_thr = 0.f, it_ipi = 0.f;
+        float c_Dx = 0.f, c_Dy = 0.f, c_Dz = 0.f, c_thr = 0.f, c_ipi = 0.f;
+        for (;;) {
+            // ---- screen until 32 survivors are queued (in either ring) or the items run out ----
+            while (qn < 32 && (!MIXED || qn32 < 32)) {
+                if (!have) {
+                    if (imask == 0) {
+                        if (ebase >= nitems) { items_done = true; break; }
+                        const int e = ebase + lane;
+                        ebase += 32 * NW;
+                        it_cnt = 0;
+                        if (e < nitems) {
+                            const int ib = e / nimg, t = e - ib * nimg;
+                            const int i = b0 + ib;
+                            const float4 b4 = __ldg(K.q4 + i);                     // (P - mu).xyz, lb
+                            const float ipi = __ldg(K.ipf + i);
+                            const float thr = b4.w + __ldg(p.lnProw + __ldg(K.shB + i)) - ln_tau;
+                            const float Dx = b4.x + sC[t], Dy = b4.y + sC[NIMG_K + t], Dz = b4.z + sC[2 * NIMG_K + t];
+                            const float dist = sqrtf(Dx * Dx + Dy * Dy + Dz * Dz);   // |P - (nu + T)|
+                            const float dlb = fmaxf(dist * (1.f - 4e-6f) - kext - 1e-4f, 0.f);
+                            const float need = __fdividef(dlb * dlb, ipi + kiqmax + iw2) - thr - 2.f * M;
+                            if (need < lbmax_ket) {                                // the strongest ket could survive
+                                it_cnt = count_above_sorted(kq4, nk_eff, need);    // kets sorted by bound
+                                it_ibt = ib | (t << 16); it_Dx = Dx; it_Dy = Dy; it_Dz = Dz;
+                                it_thr = thr; it_ipi = ipi;
+                            }
+                        }
+                        imask = __ballot_sync(0xffffffffu, it_cnt > 0);
+                        continue;
+                    }
+                    const int src = __ffs(imask) - 1;
+                    imask &= imask - 1;
+                    c_ibt = __shfl_sync(0xffffffffu, it_ibt, src);
+                    c_Dx = __shfl_sync(0xffffffffu, it_Dx, src);
+                    c_Dy = __shfl_sync(0xffffffffu, it_Dy, src);
+                    c_Dz = __shfl_sync(0xffffffffu, it_Dz, src);
+                    c_thr = __shfl_sync(0xffffffffu, it_thr, src);
+                    c_ipi = __shfl_sync(0xffffffffu, it_ipi, src);
+                    c_cnt = __shfl_sync(0xffffffffu, it_cnt, src);
+                    jpos = 0;
+                    have = true;
+                }
+                if (jpos >= c_cnt) { have = false; continue; }
+                const int jj = jpos + lane;
+                jpos += 32;
+                bool pass = false, lo32 = false;
+                if (jj < c_cnt) {
+                    const float4 k4 = __ldg(kq4 + jj);                            // (Q - nu).xyz, lb
+                    const float iq = __ldg(kipf + jj);
+                    const float ex = k4.x - c_Dx, ey = k4.y - c_Dy, ez = k4.z - c_Dz;   // Q + T - P
+                    const float r2 = ex * ex + ey * ey + ez * ez;
+                    const float isum = c_ipi + iq + iw2;
+                    pass = (c_thr + k4.w + M) * isum > r2 && r2 <= rcut2f;
+                    ++ncand;
+                    if (pass) {                                                   // max |P'| over the shell block (L819)
+                        const int i = b0 + (c_ibt & 0xffff);
+                        const float lbsum = __ldg(&K.q4[i].w) + k4.w +
+                                            __ldg(p.lnPblk + (size_t)__ldg(K.shB + i) * ns + __ldg(kshB + jj));
+                        pass = (lbsum - ln_tau + M) * isum > r2;
+                        if constexpr (MIXED)
+                            lo32 = pass && lbsum < p.ln_switch && __ldg(K.rng + i) + __ldg(K.rng + k0 + jj) < 60.f;
+                    }
+                }
+                if constexpr (MIXED) {
+                    const unsigned m32 = __ballot_sync(0xffffffffu, lo32), m64 = __ballot_sync(0xffffffffu, pass && !lo32);
+                    if (lo32) queue32[(head32 + qn32 + __popc(m32 & ltmask)) & (KQ - 1)] = make_int2((c_ibt & 0xffff) | (jj << 16), c_ibt >> 16);
+                    else if (pass) queue[(head + qn + __popc(m64 & ltmask)) & (KQ - 1)] = make_int2((c_ibt & 0xffff) | (jj << 16), c_ibt >> 16);
+                    qn32 += __popc(m32);
+                    qn += __popc(m64);
+                } else {
+                    const unsigned m = __ballot_sync(0xffffffffu, pass);
+                    if (pass) queue[(head + qn + __popc(m & ltmask)) & (KQ - 1)] = make_int2((c_ibt & 0xffff) | (jj << 16), c_ibt >> 16);
+                    qn += __popc(m);
+                }
+                __syncwarp();
+            }
+            // a partly filled ring is evaluated only when this chunk's items are exhausted (its image indices
+            // refer to the current list)
+            const bool w64 = qn >= 32 || (items_done && qn > 0);
+            const bool w32 = MIXED && (qn32 >= 32 || (items_done && qn32 > 0));
+            if (LOCKSTEP) {
+                // the evaluators of the high classes are 10-60 thousand instructions of straight-line code, far more
+                // than the instruction caches hold; the warps of a CTA therefore enter the evaluator together and
+                // share the fetched lines.  Every warp passes these barriers once per round until no warp has
+                // anything to evaluate.
+                const int any64 = __syncthreads_or(w64);
+                const int any32 = MIXED ? __syncthreads_or(w32) : 0;
+                if (!any64 && !any32) break;
+            } else if (!w64 && !w32) break;
+            // ---- evaluation: one primitive quartet-image per lane, oldest survivors first ----
+            if (w64) {
+                const int take = qn < 32 ? qn : 32;
+                int i = b0, j = k0, t = 0;
+                if (lane < take) {
+                    const int2 e = queue[(head + lane) & (KQ - 1)];
+                    i = b0 + (e.x & 0xffff); j = k0 + (int)((unsigned)e.x >> 16); t = e.y;
+                }
+                const long long eo = __ldg(K.eoff + i);
+                const double *__restrict__ bE = K.etab + eo;
+                if (lane < take) {
+                    const double X = __ldg(K.Px + j) + sT[t] - __ldg(K.Px + i), Y = __ldg(K.Py + j) + sT[NIMG_K + t] - __ldg(K.Py + i),
+                                 Z = __ldg(K.Pz + j) + sT[2 * NIMG_K + t] - __ldg(K.Pz + i);
+                    const double pb = __ldg(K.p + i), q = __ldg(K.p + j);
+                    const double r2 = X * X + Y * Y + Z * Z;
+                    const double s = rsqrt(pb + q);
+                    const double alpha = pb * q * s * s;
+                    const double th = lat.omega * rsqrt(alpha + lat.omega2);
+                    const double alpha_w = alpha * th * th;
+                    const double pref = r2 <= p.rcut2 ? __ldg(K.coef + i) * __ldg(K.coef + j) * s : 0.0;
+                    const double *__restrict__ Pb = p.Pp + (size_t)__ldg(K.aoB + i) * p.ldP + __ldg(K.aoB + j);
+                    double Rm[L + 1];
+                    boys_merged<L, double>(p.boys, r2, alpha, alpha_w, th, pref, Rm);
+                    Ev::template run<32, double>(bE, K.etab + __ldg(K.eoff + j), Pb, p.ldP, Rm, X, Y, Z, Rs, Kacc);
+                }
+                head = (head + take) & (KQ - 1);
+                qn -= take;
+                nquart += take;
+                __syncwarp();
+            }
+            if constexpr (MIXED) if (w32) {
+                const int take = qn32 < 32 ? qn32 : 32;
+                int i = b0, j = k0, t = 0;
+                if (lane < take) {
+                    const int2 e = queue32[(head32 + lane) & (KQ - 1)];
+                    i = b0 + (e.x & 0xffff); j = k0 + (int)((unsigned)e.x >> 16); t = e.y;
+                }
+                const long long eo = __ldg(K.eoff + i);
+                const float *__restrict__ bE = K.etabf + eo;
+                if (lane < take) {
+                    const double Xd = __ldg(K.Px + j) + sT[t] - __ldg(K.Px + i), Yd = __ldg(K.Py + j) + sT[NIMG_K + t] - __ldg(K.Py + i),
+                                 Zd = __ldg(K.Pz + j) + sT[2 * NIMG_K + t] - __ldg(K.Pz + i);
+                    const float X = (float)Xd, Y = (float)Yd, Z = (float)Zd;
+                    const float pb = (float)__ldg(K.p + i), q = (float)__ldg(K.p + j);
+                    const float r2 = X * X + Y * Y + Z * Z;
+                    const float s = rsqrtf(pb + q);
+                    const float alpha = pb * q * s * s;
+                    const float th = (float)lat.omega * rsqrtf(alpha + (float)lat.omega2);
+                    const float alpha_w = alpha * th * th;
+                    const float pref = Xd * Xd + Yd * Yd + Zd * Zd <= p.rcut2 ? (float)(__ldg(K.coef + i) * __ldg(K.coef + j)) * s : 0.f;
+                    const float *__restrict__ Pb = p.Ppf + (size_t)__ldg(K.aoB + i) * p.ldP + __ldg(K.aoB + j);
+                    float Rm[L + 1];
+                    boys_merged<L, float>(p.boys, r2, alpha, alpha_w, th, pref, Rm);
+                    float K32[NA * ND];
+#pragma unroll
+                    for (int c = 0; c < NA * ND; ++c) K32[c] = 0.f;
+                    Ev::template run<32, float>(bE, K.etabf + __ldg(K.eoff + j), Pb, p.ldP, Rm, X, Y, Z,
+                                                          reinterpret_cast<float *>(smem + (size_t)w * nherm(L) * 32) + lane, K32);
+#pragma unroll
+                    for (int c = 0; c < NA * ND; ++c) Kacc[c] += (double)K32[c];      // fp64 accumulation (reading C-22)
+                }
+                head32 = (head32 + take) & (KQ - 1);
+                qn32 -= take;
+                nquart32 += take;
+                __syncwarp();
+            }
         }
-        head = (head + take) & (KQ - 1);
-        qn -= take;
-        nquart += take;
-        __syncwarp();
     }
     // warp shuffle reduction, then shared-memory reduction across the CTA's warps
 #pragma unroll
@@ -260,20 +354,26 @@ sr_k_kernel(SRParams p, const int2 *__restrict__ blocks, int nblocks)
     if (lane == 0) {
         constexpr int cls = ((LA * 3 + LB) * 3 + LC) * 3 + LD;
         atomicAdd(p.counters + CNT_CAND_K + cls, c);
-        atomicAdd(p.counters + CNT_Q_K + cls, nquart);
+        atomicAdd(p.counters + CNT_Q_K + cls, nquart + nquart32);
+        if constexpr (MIXED) atomicAdd(p.counters + CNT_Q32_K + cls, nquart32);
     }
 }
 
-template <int LA, int LB, int LC, int LD>
+template <int LA, int LB, int LC, int LD, bool MIXED>
 void launch_sr_k_class(const SRParams &p, const int2 *blocks, int nblocks, cudaStream_t st)
 {
-    constexpr size_t smem = k_smem_bytes<LA, LB, LC, LD>();
-    static bool attr_set = false;
-    if (!attr_set) {
-        cudaFuncSetAttribute(sr_k_kernel<LA, LB, LC, LD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        attr_set = true;
-    }
-    sr_k_kernel<LA, LB, LC, LD><<<nblocks, k_nthreads(LA + LB + LC + LD), smem, st>>>(p, blocks, nblocks);
+    constexpr size_t smem = k_smem_bytes<LA, LB, LC, LD, MIXED>();
+    const int grid = p.shard_n > 1 ? (nblocks + p.shard_n - 1) / p.shard_n : nblocks;
+    if (grid <= 0) return;
+    sr_k_kernel<LA, LB, LC, LD, MIXED><<<grid, k_nthreads(LA + LB + LC + LD), smem, st>>>(p, blocks, nblocks);
+}
+
+// the attribute is per device: pbc_jk_create calls this for the handle's device
+template <int LA, int LB, int LC, int LD, bool MIXED>
+void set_sr_k_attr()
+{
+    cudaFuncSetAttribute(sr_k_kernel<LA, LB, LC, LD, MIXED>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                         (int)k_smem_bytes<LA, LB, LC, LD, MIXED>());
 }
 
 }  // namespace pbcjk

@@ -13,7 +13,8 @@ namespace pbcjk {
 void CAT(launch_sr_j_, J_LB)(int LK, const SRParams &p, const int *bra_idx, int nbra, cudaStream_t st)
 {
     if (nbra <= 0) return;
-    dim3 grid((nbra + 3) / 4), block(128);
+    const int mine = p.shard_n > 1 ? (nbra + p.shard_n - 1) / p.shard_n : nbra;     // bras of this rank (multi-GPU)
+    dim3 grid((mine + 3) / 4), block(128);
     switch (LK) {
     case 0: sr_j_kernel<J_LB, 0><<<grid, block, 0, st>>>(p, bra_idx, nbra); break;
     case 1: sr_j_kernel<J_LB, 1><<<grid, block, 0, st>>>(p, bra_idx, nbra); break;

@@ -378,3 +378,51 @@ def test_sampled_blocks_equal_full(oracle_mod, pd_ref):
     for key in ("J", "K", "J_sr", "K_sr", "J_lr", "K_lr", "J_self", "K_self"):
         assert np.max(np.abs(rs[key][m] - r[key][m])) < 1e-13, key
         assert np.all(rs[key][~m] == 0.0)
+
+
+# ---------------------------------------------------------------- P13: eq 5-6 normalisation of p and d components
+def _quad_1d(m, c):
+    """int_{-inf}^{inf} x^m e^{-c x^2} dx by adaptive quadrature (no closed form typed in)"""
+    return mp.quad(lambda x: x ** m * mp.exp(-c * x * x), [-mp.inf, 0, mp.inf])
+
+
+def test_prim_norm_by_quadrature(oracle_mod):
+    """prim_norm (eq 5-6, reading C-1) pinned without retyping eq 6: a primitive is "normalised" iff
+    int phi^2 = 1, so N = (int [x^i y^j z^k e^{-a r^2}]^2)^{-1/2} with the integral taken by mpmath quadrature.
+    One centre with uncontracted s, p and d shells (coefficient 1) in a 40-bohr cube, where lattice images do not
+    overlap (e^{-0.45 * 40^2} underflows): the oracle's crystalline S (eq 21) must equal the matrix of quadrature
+    overlaps of the quadrature-normalised functions, for every one of the 10 components incl. d_xy, d_xz, d_yz."""
+    mp.mp.dps = 30
+    exps = {0: 1.3, 1: 0.9, 2: 1.1}
+    wl = W.Workload(name="norm_pin", cell=np.eye(3) * 40.0, xyz=np.array([[1.0, -2.0, 0.5]]),
+                    sh_atom=np.zeros(3, np.int32), sh_l=np.array([0, 1, 2], np.int32), sh_nprim=np.ones(3, np.int32),
+                    sh_off=np.arange(3, dtype=np.int32), exps=np.array([exps[0], exps[1], exps[2]]),
+                    coefs=np.ones(3), omega=0.3, n_occ=1, seed=1)
+    S = oracle_mod.overlap(wl)
+    comps = [(0, (0, 0, 0))] + [(1, c) for c in [(1, 0, 0), (0, 1, 0), (0, 0, 1)]] + \
+            [(2, c) for c in [(2, 0, 0), (1, 1, 0), (1, 0, 1), (0, 2, 0), (0, 1, 1), (0, 0, 2)]]     # C-10 order
+    assert S.shape == (10, 10)
+
+    def raw(ci, cj):
+        (li, pi), (lj, pj) = ci, cj
+        c = exps[li] + exps[lj]
+        return _quad_1d(pi[0] + pj[0], c) * _quad_1d(pi[1] + pj[1], c) * _quad_1d(pi[2] + pj[2], c)
+
+    nrm = [1 / mp.sqrt(raw(c, c)) for c in comps]
+    for i, ci in enumerate(comps):
+        for j, cj in enumerate(comps):
+            ref = float(nrm[i] * nrm[j] * raw(ci, cj))
+            assert abs(S[i, j] - ref) < 2e-14, (ci, cj, S[i, j], ref)
+    assert np.abs(np.diag(S) - 1.0).max() < 2e-14
+    # two values the quadrature must have produced (textbook): <d_xx|d_yy> = 1/3, <d_xy|d_xy> = 1
+    assert abs(S[4, 7] - 1.0 / 3.0) < 1e-14 and abs(S[5, 5] - 1.0) < 2e-14
+
+
+def test_pd_test_unit_diagonal_in_scaled_cell(oracle_mod):
+    """Every component of the s/p/d test cell has unit crystalline self-overlap once the cell is scaled (x6) so that
+    images do not overlap -- for the uncontracted shells directly by eq 5-6, for the contracted ones through C-9
+    (axis-aligned component scaled to unit local self-overlap; d_xy... follow from the per-component norm)."""
+    wl = W.pd_test_cell(L=36.0)
+    S = oracle_mod.overlap(wl)
+    assert wl.nbf == 14
+    assert np.abs(np.diag(S) - 1.0).max() < 1e-13

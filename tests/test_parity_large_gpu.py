@@ -25,8 +25,9 @@ def torch_cuda():
 
 
 def _sample_blocks(wl, nblk, seed):
-    """Seeded output shell blocks, cycling over the (l_mu, l_nu) classes of the workload; half of them
-    between shells of neighbouring atoms (large elements), half anywhere in the cell."""
+    """Seeded output shell blocks, cycling over the (l_mu, l_nu) classes of the workload: per class in turn a block
+    between shells of neighbouring atoms (large elements), one anywhere in the cell, and the FARTHEST-separated pair
+    (minimum image) -- the blocks where a too eager screen would show first."""
     rng = np.random.default_rng(seed)
     by_l = {}
     for s, l in enumerate(wl.sh_l):
@@ -39,12 +40,13 @@ def _sample_blocks(wl, nblk, seed):
         la, lb = classes[k % len(classes)]
         mu = int(rng.choice(by_l[la]))
         cand = by_l[lb]
-        if k % 2 == 0:       # nearest few atoms (minimum image)
+        kind = (k // len(classes)) % 3
+        if kind in (0, 2):   # nearest few atoms / the farthest one (minimum image)
             d = wl.xyz[wl.sh_atom[cand]] - wl.xyz[wl.sh_atom[mu]]
             f = d @ inv
             d = (f - np.round(f)) @ wl.cell
             order = np.argsort(np.linalg.norm(d, axis=1), kind="stable")
-            nu = int(cand[int(order[int(rng.integers(0, min(12, len(order))))])])
+            nu = int(cand[int(order[int(rng.integers(0, min(12, len(order))))])]) if kind == 0 else int(cand[int(order[-1])])
         else:
             nu = int(rng.choice(cand))
         blocks.append((mu, nu))
@@ -78,7 +80,7 @@ def _case(oracle_mod, name):
     return _CACHE[name]
 
 
-@pytest.mark.parametrize("name,nblk", [("si64", 9), ("water64", 9), ("water343", 4)])
+@pytest.mark.parametrize("name,nblk", [("si64", 27), ("water64", 27), ("water343", 12)])
 def test_sampled_blocks_real_space(torch_cuda, oracle_mod, name, nblk):
     wl, S, P = _case(oracle_mod, name)
     blocks = _sample_blocks(wl, nblk, seed=4242)
@@ -92,6 +94,67 @@ def test_sampled_blocks_real_space(torch_cuda, oracle_mod, name, nblk):
     assert np.abs(ref["J_sr"][m]).max() > 1e-6 and np.abs(ref["K_sr"][m]).max() > 1e-9
     assert dJ < TOL, (name, dJ)
     assert dK < TOL, (name, dK)
+
+
+def test_config5_reciprocal_space_and_invariants(torch_cuda, oracle_mod):
+    """Config 5 (water343, N = 4459): its reciprocal-space path runs another batch geometry than the smaller configs
+    (37 G vectors per batch, 12.8 GB stacks).  (a) LR + SELF of sampled blocks against the oracle with the G sum
+    truncated at |G| <= 0.32 on both sides (the oracle needs seconds per G at this size); (b) ONE full-size build with a
+    rank-1 density P = c c^T -- the factor of P has rank 1, so the dense contraction is cheap while every G batch, the
+    ragged last batch and the whole real-space part run at full size: symmetry and J c = K c (P8)."""
+    wl, S, P = _case(oracle_mod, "water343")
+    blocks = _sample_blocks(wl, 6, seed=77)
+    ref = oracle_mod.jk(wl, P, blocks=blocks, parts="lr+self", g_cut=0.32)
+    assert ref["counts"]["n_G"] >= 30
+    m = oracle_mod.block_mask(wl, blocks)
+    J, K, st = _build(torch_cuda, wl, P, parts="lr+self", g_cut=0.32)
+    assert 2 * st["n_g"] == ref["counts"]["n_G"]
+    assert np.abs(J - (ref["J_lr"] + ref["J_self"]))[m].max() < TOL
+    assert np.abs(K - (ref["K_lr"] + ref["K_self"]))[m].max() < TOL
+    rng = np.random.default_rng(5)
+    c = rng.standard_normal(wl.nbf)
+    c /= np.sqrt(c @ S @ c)
+    J1, K1, st1 = _build(torch_cuda, wl, np.outer(c, c))
+    assert st1["n_g"] > 10000
+    assert np.abs(J1 - J1.T).max() < 1e-11 and np.abs(K1 - K1.T).max() < 1e-11
+    assert np.abs(J1 @ c - K1 @ c).max() < TOL * 10
+    assert 0.5 * c @ J1 @ c > 0.0
+
+
+def test_outermost_g_shell_full_size(torch_cuda, oracle_mod):
+    """The high-|G| end of the reciprocal-space sum at full N (water64): only G with g_min <= |G| < g_cut on both sides
+    (selection only).  There the weight exp(-G^2/4w^2) has fallen to ~1e-14 and the (-iG)^t polynomial reaches G^4, so
+    the comparison is relative to the size of that window's contribution."""
+    wl, S, P = _case(oracle_mod, "water64")
+    blocks = _sample_blocks(wl, 6, seed=5)
+    g_min, g_cut = 3.37, 3.41          # 3.41 = 2 w sqrt(ln 1e14): the library's default cutoff for this config
+    ref = oracle_mod.jk(wl, P, blocks=blocks, parts="lr", g_min=g_min, g_cut=g_cut)
+    assert 100 <= ref["counts"]["n_G"] <= 600, ref["counts"]["n_G"]
+    m = oracle_mod.block_mask(wl, blocks)
+    J, K, st = _build(torch_cuda, wl, P, parts="lr", g_min=g_min, g_cut=g_cut)
+    assert 2 * st["n_g"] == ref["counts"]["n_G"]
+    scale = max(np.abs(ref["J_lr"][m]).max(), np.abs(ref["K_lr"][m]).max())
+    assert scale > 0.0
+    print(f"outermost G shell: {ref['counts']['n_G']} vectors, largest element {scale:.3e}")
+    assert np.abs(J - ref["J_lr"])[m].max() < 1e-6 * scale       # relative: the window's own contribution is ~1e-14
+    assert np.abs(K - ref["K_lr"])[m].max() < 1e-6 * scale
+    assert np.abs(J - ref["J_lr"])[m].max() < TOL and np.abs(K - ref["K_lr"])[m].max() < TOL
+
+
+def test_mixed_precision_sampled_blocks_water64(torch_cuda, oracle_mod):
+    """Config 4 in mixed precision (north_star: <= 1e-6 Eh vs the fp64 oracle, reported separately): real-space part of
+    sampled output blocks of the full build."""
+    wl, S, P = _case(oracle_mod, "water64")
+    blocks = _sample_blocks(wl, 9, seed=4242)
+    ref = oracle_mod.jk(wl, P, blocks=blocks, parts="sr")
+    m = oracle_mod.block_mask(wl, blocks)
+    J, K, st = _build(torch_cuda, wl, P, parts="sr", precision=1)
+    dJ = np.abs(J - ref["J_sr"])[m].max()
+    dK = np.abs(K - ref["K_sr"])[m].max()
+    share = st["quartets_k_fp32"] / st["quartets_k"]
+    print(f"mixed precision water64: max|dJ| = {dJ:.3e}, max|dK| = {dK:.3e}, fp32 share of K quartets = {share:.3f}")
+    assert share > 0.2
+    assert dJ < TOL and dK < 1e-6
 
 
 @pytest.mark.parametrize("name", ["si64", "water64"])
