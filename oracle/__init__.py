@@ -50,6 +50,7 @@ def _load():
         _lib.orc_jk.restype = C.c_int
         _lib.orc_nbf.restype = C.c_int
         _lib.orc_num_threads.restype = C.c_int
+        _lib.orc_one_electron.restype = C.c_int
     return _lib
 
 
@@ -159,6 +160,32 @@ def jk(wl, P: np.ndarray, omega: Optional[float] = None, blocks: Optional[Sequen
                 K_sr=Ksr, K_lr=Klr, K_self=Kself, S=S,
                 counts=dict(quartets_J=int(counts[0]), quartets_K=int(counts[1]),
                             pair_images=int(counts[2]), n_G=int(counts[3])))
+
+
+def one_electron(wl, charges, omega: Optional[float] = None, delta_o: float = 1e-18, r_cut: Optional[float] = None,
+                 g_cut: Optional[float] = None) -> dict:
+    """One-electron Ewald terms: kinetic matrix T (SI eq S1), the interaction V of every pair density
+    with the point charges `charges` (one per atom; PAPER eq 52, SR / LR / SELF parts) under the zero-mean periodic
+    kernel, and the Ewald energy E_nuc of the point charges themselves (eq 91)."""
+    lib = _load()
+    s = _Sys(wl)
+    n = lib.orc_nbf(C.byref(s.c))
+    q = np.ascontiguousarray(charges, dtype=np.float64)
+    assert q.shape == (s.c.natom,)
+    o = _Opts()
+    o.delta_o = delta_o
+    o.r_cut = float(wl.r_cut if r_cut is None else r_cut)
+    o.g_cut = float(wl.g_cut if g_cut is None else g_cut)
+    o.which, o.parts, o.g_min = 3, 7, 0.0
+    om = float(wl.omega if omega is None else omega)
+    z = lambda: np.zeros((n, n))
+    T, Vsr, Vlr, Vself = z(), z(), z(), z()
+    e = np.zeros(4)
+    rc = lib.orc_one_electron(C.byref(s.c), C.c_double(om), C.byref(o), _dp(q), _dp(T), _dp(Vsr), _dp(Vlr), _dp(Vself), _dp(e))
+    if rc != 0:
+        raise RuntimeError("oracle failed")
+    return dict(T=T, V=Vsr + Vlr + Vself, V_sr=Vsr, V_lr=Vlr, V_self=Vself, E_nuc=float(e[3]),
+                E_nuc_parts=dict(lr=float(e[0]), sr=float(e[1]), const=float(e[2])))
 
 
 def block_mask(wl, blocks: Sequence[Tuple[int, int]]) -> np.ndarray:

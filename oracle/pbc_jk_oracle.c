@@ -24,6 +24,9 @@
  * C-4 (sign and s-index of eq 98's real-space term), C-6 (SELF kept), C-10
  * (component order p: x,y,z; d: xx,xy,xz,yy,yz,zz).
  *
+ * One-electron Ewald terms (orc_one_electron below): kinetic matrix (SI eq S1), nuclear
+ * attraction matrix (eq 52), nuclear repulsion energy (eq 91); reading C-27 for the garbled eq S1.
+ *
  * Pins (tests/test_oracle_pins.py): closed-form attenuated (ss|ss) with erf,
  * 1F1 Boys values, pure reciprocal-space brute force, omega invariance,
  * Madelung constants, symmetry, rank-1 J/K identity, positivity, geometric
@@ -792,6 +795,202 @@ int orc_jk(const orc_system *s, double omega, const orc_opts *o, const double *P
         }
     }
     free(S); free(bm); free(bn); free_pair_list(&pl);
+    return 0;
+}
+
+/* ------------------------------------------------------------------ */
+/* One-electron Ewald terms: kinetic matrix, nuclear     */
+/* attraction matrix, nuclear repulsion energy.  Gamma point.            */
+/* ------------------------------------------------------------------ */
+
+/* E^{ij}_0 ... of one direction for i <= la, j <= lb (eq 17-20), any la, lb: the kinetic integral needs j up to l + 2 */
+static void hermite_E_n(int la, int lb, double a, double b, double Ax, double Bx, int dj, int dt, double *E /* [la+1][dj][dt] */)
+{
+    double p = a + b, mu = a * b / p;
+    double Px = (a * Ax + b * Bx) / p;
+    double XPA = Px - Ax, XPB = Px - Bx;
+#define EE(i, j, t) E[((i) * dj + (j)) * dt + (t)]
+    for (int i = 0; i <= la; ++i) for (int j = 0; j < dj; ++j) for (int t = 0; t < dt; ++t) EE(i, j, t) = 0.0;
+    EE(0, 0, 0) = exp(-mu * (Ax - Bx) * (Ax - Bx));                                  /* eq 19 */
+    for (int i = 0; i < la; ++i)                                                     /* eq 17 */
+        for (int t = 0; t <= i + 1; ++t) {
+            double v = XPA * (t <= i ? EE(i, 0, t) : 0.0);
+            if (t > 0) v += EE(i, 0, t - 1) / (2.0 * p);
+            if (t + 1 <= i) v += (t + 1) * EE(i, 0, t + 1);
+            EE(i + 1, 0, t) = v;
+        }
+    for (int i = 0; i <= la; ++i)                                                    /* eq 18 */
+        for (int j = 0; j < lb; ++j)
+            for (int t = 0; t <= i + j + 1; ++t) {
+                double v = XPB * (t <= i + j ? EE(i, j, t) : 0.0);
+                if (t > 0) v += EE(i, j, t - 1) / (2.0 * p);
+                if (t + 1 <= i + j) v += (t + 1) * EE(i, j, t + 1);
+                EE(i, j + 1, t) = v;
+            }
+#undef EE
+}
+
+/*
+ * T (SI eq S1): T_mn = sum_{R,prims} C_m C_n (pi/p)^{3/2} t_local, with per direction
+ *   k_tau = -j(j-1)/2 E^{i,j-2}_0 + (2j+1) b E^{i,j}_0 - 2 b^2 E^{i,j+2}_0     (-1/2 d^2/dx^2 acting on the second function)
+ *   t_local = k_x E_0y E_0z + E_0x k_y E_0z + E_0x E_0y k_z.
+ * Reading C-27: PAPER.md prints the x bracket in full; the y and z brackets are garbled (the -2b^2 E^{j+2} term is
+ * detached and repeated).  The Laplacian treats the three directions alike, so the x bracket is used for each.
+ *
+ * V (eq 52), per point charge q_C at C, L = C - P + R_C (so that the sign (-1)^{|t|} of reading C-4 applies):
+ *   SR   = q_C C_m C_n (2 pi/p) sum_{R_C} sum_t (-1)^{|t|} E_t [ R^0_t(p, L) - theta R^0_t(a_w, L) ],
+ *          theta = w/sqrt(p + w^2), a_w = p w^2/(p + w^2)
+ *   LR   = sum_{G != 0} 4 pi/(Omega G^2) e^{-G^2/4w^2} Re[ conj(rho_mn(G)) q_C e^{-iG.C} ]
+ *   SELF = -pi/(Omega w^2) S_mn q_C
+ * Sign convention of the paper: V_mnC is the Coulomb interaction of the pair density with a charge +q_C under the
+ * zero-mean periodic kernel; the electron-nucleus attraction matrix is -V with q_C = Z_C.
+ *
+ * E_nuc (eq 91); enuc[0] = reciprocal part, [1] = real-space part, [2] = constant terms, [3] = total.
+ */
+int orc_one_electron(const orc_system *s, double omega, const orc_opts *o, const double *charge /* natom */,
+                     double *T, double *Vsr, double *Vlr, double *Vself, double *enuc)
+{
+    pair_list pl; build_pair_list(s, o->delta_o, o->r_cut, &pl);
+    int N = pl.nbf;
+    size_t NN = (size_t)N * N;
+    memset(T, 0, 8 * NN); memset(Vsr, 0, 8 * NN); memset(Vlr, 0, 8 * NN); memset(Vself, 0, 8 * NN);
+    double *S = malloc(8 * NN); overlap_from_list(s, &pl, S);
+    double qtot = 0.0; for (int c = 0; c < s->natom; ++c) qtot += charge[c];
+    double w2 = omega * omega;
+    /* ---- kinetic ---- */
+    for (int ip = 0; ip < pl.n; ++ip) {
+        const pair_img *pi = &pl.v[ip];
+        const prim_pair *pp = &pi->pp;
+        int la = pp->la, lb = pp->lb;
+        enum { DJ = LMAX + 3, DT = 2 * LMAX + 3 };
+        double E[3][(LMAX + 1) * DJ * DT];
+        for (int k = 0; k < 3; ++k) hermite_E_n(la, lb + 2, pp->a, pp->b, pp->A[k], pp->B[k], DJ, DT, E[k]);
+#define E0(k, i, j) ((j) < 0 ? 0.0 : E[k][((i) * DJ + (j)) * DT])
+        double Ca[6], Cb[6];
+        comp_coefs(pi->ca, pp->a, la, Ca); comp_coefs(pi->cb, pp->b, lb, Cb);
+        double g = pow(M_PI / pp->p, 1.5), b = pp->b;
+        for (int ka = 0; ka < ncart(la); ++ka)
+            for (int kb = 0; kb < ncart(lb); ++kb) {
+                int ca[3], cb[3];
+                cart_comp(la, ka, &ca[0], &ca[1], &ca[2]); cart_comp(lb, kb, &cb[0], &cb[1], &cb[2]);
+                double e0[3], kk[3];
+                for (int k = 0; k < 3; ++k) {
+                    int i = ca[k], j = cb[k];
+                    e0[k] = E0(k, i, j);
+                    kk[k] = -0.5 * j * (j - 1) * E0(k, i, j - 2) + (2 * j + 1) * b * E0(k, i, j) - 2.0 * b * b * E0(k, i, j + 2);
+                }
+                double t = kk[0] * e0[1] * e0[2] + e0[0] * kk[1] * e0[2] + e0[0] * e0[1] * kk[2];
+                T[(size_t)(pl.ao_off[pi->shA] + ka) * N + pl.ao_off[pi->shB] + kb] += Ca[ka] * Cb[kb] * g * t;
+            }
+#undef E0
+    }
+    /* ---- V, short range ---- */
+#pragma omp parallel for schedule(dynamic, 8)
+    for (int ip = 0; ip < pl.n; ++ip) {
+        const pair_img *pi = &pl.v[ip];
+        const prim_pair *pp = &pi->pp;
+        int la = pp->la, lb = pp->lb, Lb = la + lb;
+        double p = pp->p;
+        double theta = omega / sqrt(p + w2), aw = p * w2 / (p + w2);
+        double Ca[6], Cb[6];
+        comp_coefs(pi->ca, pp->a, la, Ca); comp_coefs(pi->cb, pp->b, lb, Cb);
+        double acc[36]; for (int k = 0; k < 36; ++k) acc[k] = 0.0;
+        for (int c = 0; c < s->natom; ++c) {
+            if (charge[c] == 0.0) continue;
+            double C1e = fabs(charge[c]) * pi->bound * 2.0 * M_PI / p;               /* eq 42 prefactor */
+            double arg = C1e * (1.0 - theta) / o->delta_o;
+            if (arg <= 1.0) continue;
+            double r = sqrt((1.0 / p + 1.0 / w2) * log(arg));                        /* eq 43 */
+            if (o->r_cut > 0 && r > o->r_cut) r = o->r_cut;
+            const double *Cc = s->xyz + 3 * c;
+            double ctr[3] = { pp->P[0] - Cc[0], pp->P[1] - Cc[1], pp->P[2] - Cc[2] };
+            double *Tl; int nT = translations_in_sphere(s->cell, pl.bvec, ctr, r, &Tl, NULL);
+            for (int k = 0; k < nT; ++k) {
+                double Lv[3] = { Cc[0] + Tl[3 * k] - pp->P[0], Cc[1] + Tl[3 * k + 1] - pp->P[1], Cc[2] + Tl[3 * k + 2] - pp->P[2] };
+                rtab R;
+                for (int t = 0; t <= Lb; ++t) for (int u = 0; u <= Lb; ++u) for (int v = 0; v <= Lb; ++v) R[t][u][v] = 0.0;
+                hermite_R_add(Lb, p, Lv, 1.0, R);
+                hermite_R_add(Lb, aw, Lv, -theta, R);
+                for (int ka = 0; ka < ncart(la); ++ka)
+                    for (int kb = 0; kb < ncart(lb); ++kb) {
+                        int ca[3], cb[3];
+                        cart_comp(la, ka, &ca[0], &ca[1], &ca[2]); cart_comp(lb, kb, &cb[0], &cb[1], &cb[2]);
+                        double sum = 0.0;
+                        for (int t = 0; t <= ca[0] + cb[0]; ++t)
+                            for (int u = 0; u <= ca[1] + cb[1]; ++u)
+                                for (int v = 0; v <= ca[2] + cb[2]; ++v)
+                                    sum += (((t + u + v) & 1) ? -1.0 : 1.0) * E3(pp, ca, cb, t, u, v) * R[t][u][v];
+                        acc[ka * ncart(lb) + kb] += charge[c] * sum;
+                    }
+            }
+            free(Tl);
+        }
+        for (int ka = 0; ka < ncart(la); ++ka)
+            for (int kb = 0; kb < ncart(lb); ++kb) {
+                double v = Ca[ka] * Cb[kb] * (2.0 * M_PI / p) * acc[ka * ncart(lb) + kb];
+#pragma omp atomic
+                Vsr[(size_t)(pl.ao_off[pi->shA] + ka) * N + pl.ao_off[pi->shB] + kb] += v;
+            }
+    }
+    /* ---- V, long range; E_nuc reciprocal part ---- */
+    double gcut = o->g_cut > 0 ? o->g_cut : 2.0 * omega * sqrt(log(1.0 / o->delta_o));
+    double zero[3] = { 0, 0, 0 };
+    double *G; int nG;
+    {
+        double acell[9]; for (int i = 0; i < 9; ++i) acell[i] = s->cell[i];
+        nG = translations_in_sphere(pl.bvec, acell, zero, gcut, &G, NULL);
+    }
+    double e_lr = 0.0;
+    for (int ig = 0; ig < nG; ++ig) {
+        const double *Gv = G + 3 * ig;
+        double G2 = Gv[0] * Gv[0] + Gv[1] * Gv[1] + Gv[2] * Gv[2];
+        if (G2 < 1e-20) continue;
+        double w = 4.0 * M_PI / (pl.vol * G2) * exp(-G2 / (4.0 * w2));
+        double nr = 0.0, ni = 0.0;                                                    /* rho_nuc(G) = sum q_C e^{-iG.C} */
+        for (int c = 0; c < s->natom; ++c) {
+            double ph = -(Gv[0] * s->xyz[3 * c] + Gv[1] * s->xyz[3 * c + 1] + Gv[2] * s->xyz[3 * c + 2]);
+            nr += charge[c] * cos(ph); ni += charge[c] * sin(ph);
+        }
+        e_lr += 0.5 * w * (nr * nr + ni * ni);          /* 1/2 sum_{A,B} q_A q_B cos(G.(A-B)), A = B included (eq 91) */
+        double re[36], im[36];
+        for (int i = 0; i < pl.n; ++i) {
+            const pair_img *pi = &pl.v[i];
+            int na = ncart(pi->pp.la), nb = ncart(pi->pp.lb);
+            pair_rho_G(pi, Gv, re, im);
+            for (int a = 0; a < na; ++a)
+                for (int b = 0; b < nb; ++b)
+                    Vlr[(size_t)(pl.ao_off[pi->shA] + a) * N + pl.ao_off[pi->shB] + b] += w * (re[a * nb + b] * nr + im[a * nb + b] * ni);
+        }
+    }
+    free(G);
+    /* ---- V, SELF ---- */
+    for (size_t k = 0; k < NN; ++k) Vself[k] = -M_PI / (pl.vol * w2) * qtot * S[k];
+    /* ---- E_nuc real-space part and constants (eq 91) ---- */
+    double e_sr = 0.0, e_c = 0.0;
+    {
+        double rb = sqrt(log(1.0 / o->delta_o)) / omega;                               /* erfc(x) < e^{-x^2}: eq 92 */
+        for (int a = 0; a < s->natom; ++a)
+            for (int b = a; b < s->natom; ++b) {
+                double d[3] = { s->xyz[3 * a] - s->xyz[3 * b], s->xyz[3 * a + 1] - s->xyz[3 * b + 1], s->xyz[3 * a + 2] - s->xyz[3 * b + 2] };
+                double md[3] = { -d[0], -d[1], -d[2] };
+                double *Tl; int nT = translations_in_sphere(s->cell, pl.bvec, md, rb, &Tl, NULL);
+                double sum = 0.0;
+                for (int k = 0; k < nT; ++k) {
+                    double v[3] = { d[0] + Tl[3 * k], d[1] + Tl[3 * k + 1], d[2] + Tl[3 * k + 2] };
+                    double r = norm3(v);
+                    if (r < 1e-12) continue;                                           /* A = B, R = 0 */
+                    sum += erfc(omega * r) / r;
+                }
+                free(Tl);
+                e_sr += (a == b ? 0.5 : 1.0) * charge[a] * charge[b] * sum;
+            }
+        double q2 = 0.0; for (int a = 0; a < s->natom; ++a) q2 += charge[a] * charge[a];
+        /* -4pi/(4 w^2 Omega) for every pair (A < B) and half of it for A = B: -pi/(Omega w^2) * qtot^2 / 2; -w/sqrt(pi) q_A^2 */
+        e_c = -M_PI / (pl.vol * w2) * 0.5 * qtot * qtot - omega / sqrt(M_PI) * q2;
+    }
+    enuc[0] = e_lr; enuc[1] = e_sr; enuc[2] = e_c; enuc[3] = e_lr + e_sr + e_c;
+    free(S);
+    free_pair_list(&pl);
     return 0;
 }
 

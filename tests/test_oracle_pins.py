@@ -426,3 +426,92 @@ def test_pd_test_unit_diagonal_in_scaled_cell(oracle_mod):
     S = oracle_mod.overlap(wl)
     assert wl.nbf == 14
     assert np.abs(np.diag(S) - 1.0).max() < 1e-13
+
+
+# ---------------------------------------------------------------- P14-P16: one-electron Ewald terms
+def test_kinetic_by_quadrature(oracle_mod):
+    """Kinetic matrix (SI eq S1, reading C-27) without the E recursion: one s, one p and one d primitive on
+    two centres 1.1 bohr apart in a 40-bohr cube (no image overlap); T_mn = -1/2 int phi_m phi_n'' separates into 1-D
+    integrals taken by mpmath quadrature, with the functions normalised by quadrature as well."""
+    mp.mp.dps = 30
+    exps = [1.3, 0.9, 1.1, 0.7]
+    ls = [0, 1, 2, 1]
+    cen = np.array([[0.3, -0.2, 0.1], [0.3 + 0.7, -0.2 + 0.6, 0.1 - 0.6]])
+    at = [0, 0, 1, 1]
+    wl = W.Workload(name="kin_pin", cell=np.eye(3) * 40.0, xyz=cen, sh_atom=np.array(at, np.int32),
+                    sh_l=np.array(ls, np.int32), sh_nprim=np.ones(4, np.int32), sh_off=np.arange(4, dtype=np.int32),
+                    exps=np.array(exps), coefs=np.ones(4), omega=0.3, n_occ=1, seed=1)
+    T = oracle_mod.one_electron(wl, np.zeros(2))["T"]
+    funcs = []                                      # (exponent, centre, (ix, iy, iz))
+    for sh in range(4):
+        for comp in pure_g.cart_components(ls[sh]):
+            funcs.append((exps[sh], cen[at[sh]], comp))
+    assert T.shape == (len(funcs), len(funcs))
+
+    def g1(x, a, c, i):
+        return (x - c) ** i * mp.exp(-a * (x - c) ** 2)
+
+    def ov(f, g, d):
+        return mp.quad(lambda x: g1(x, f[0], f[1][d], f[2][d]) * g1(x, g[0], g[1][d], g[2][d]), [-mp.inf, 0, mp.inf])
+
+    def kin(f, g, d):
+        return mp.quad(lambda x: -0.5 * g1(x, f[0], f[1][d], f[2][d]) * mp.diff(lambda y: g1(y, g[0], g[1][d], g[2][d]), x, 2),
+                       [-mp.inf, 0, mp.inf])
+
+    nrm = [1 / mp.sqrt(ov(f, f, 0) * ov(f, f, 1) * ov(f, f, 2)) for f in funcs]
+    rng = np.random.default_rng(0)
+    pairs = [(i, i) for i in range(len(funcs))] + [tuple(p) for p in rng.integers(0, len(funcs), (14, 2))]
+    for (i, j) in pairs:
+        f, g = funcs[i], funcs[j]
+        s = [ov(f, g, d) for d in range(3)]
+        k = [kin(f, g, d) for d in range(3)]
+        ref = float(nrm[i] * nrm[j] * (k[0] * s[1] * s[2] + s[0] * k[1] * s[2] + s[0] * s[1] * k[2]))
+        assert abs(T[i, j] - ref) < 1e-11 * max(1.0, abs(ref)), (i, j, T[i, j], ref)
+    assert np.abs(T - T.T).max() < 1e-13          # hermiticity: the Laplacian acts on the second function only
+
+
+def test_nuclear_attraction_pure_g_and_omega(oracle_mod):
+    """V of eq 52 (point charges under the zero-mean periodic kernel) against the plain reciprocal-space definition
+    V_mn = sum_C q_C (1/Omega) sum_{G != 0} (4 pi/G^2) Re[conj(rho_mn(G)) e^{-iG.C}] -- no Boys function, no E or R
+    recursion, no Ewald split (tests/pure_g.py) -- and its independence of the Ewald parameter."""
+    wl = W.pd_test_cell()
+    q = np.array([1.5, -0.7])                       # a charged cell on purpose: the SELF term matters
+    ref = oracle_mod.one_electron(wl, q)
+    G = pure_g.g_vectors(wl.cell, 24.0)
+    vol = abs(np.linalg.det(wl.cell))
+    V = np.zeros((wl.nbf, wl.nbf))
+    for s in range(0, G.shape[0], 16384):
+        Gc = G[s:s + 16384]
+        rho = pure_g.pair_density_ft(wl, Gc)
+        nuc = (q[None, :] * np.exp(-1j * Gc @ wl.xyz.T)).sum(1)
+        V += np.einsum("g,mng,g->mn", 4 * math.pi / (vol * (Gc * Gc).sum(1)), rho.conj(), nuc).real
+    assert np.abs(ref["V"] - V).max() < 1e-9
+    assert np.abs(ref["V"]).max() > 0.05 and np.abs(ref["V_self"]).max() > 1e-3
+    for om in (0.3, 0.9):
+        r2 = oracle_mod.one_electron(wl, q, omega=om)
+        assert np.abs(r2["V"] - ref["V"]).max() < 1e-10
+        assert abs(r2["E_nuc"] - ref["E_nuc"]) < 1e-10
+    assert np.abs(ref["V"] - ref["V"].T).max() < 1e-13
+
+
+def test_nuclear_repulsion_madelung(oracle_mod):
+    """E_nuc of eq 91 against textbook constants: one unit charge in a cube (charged cell: 1/2 xi / L) and the rock-salt
+    arrangement of +-1 charges (-8 M / L per conventional cell)."""
+    L = 7.0
+    one = W.Workload(name="q1", cell=np.eye(3) * L, xyz=np.array([[0.4, 0.1, -0.3]]), sh_atom=np.zeros(1, np.int32),
+                     sh_l=np.zeros(1, np.int32), sh_nprim=np.ones(1, np.int32), sh_off=np.zeros(1, np.int32),
+                     exps=np.array([1.0]), coefs=np.ones(1), omega=0.5, n_occ=1, seed=1)
+    e = oracle_mod.one_electron(one, np.array([1.0]))["E_nuc"]
+    assert abs(e - 0.5 * XI_CUBIC / L) < 1e-11
+    sites, ch = [], []
+    for i in range(2):
+        for j in range(2):
+            for k in range(2):
+                sites.append([i * L / 2, j * L / 2, k * L / 2]); ch.append(1.0 if (i + j + k) % 2 == 0 else -1.0)
+    n = len(sites)
+    nacl = W.Workload(name="nacl", cell=np.eye(3) * L, xyz=np.array(sites), sh_atom=np.arange(n, dtype=np.int32),
+                      sh_l=np.zeros(n, np.int32), sh_nprim=np.ones(n, np.int32), sh_off=np.arange(n, dtype=np.int32),
+                      exps=np.full(n, 2.0), coefs=np.ones(n), omega=0.45, n_occ=1, seed=1)
+    for om in (0.45, 0.8):
+        e = oracle_mod.one_electron(nacl, np.array(ch), omega=om)["E_nuc"]
+        assert abs(e - (-8.0 * M_NACL / L)) < 1e-10, (om, e)
