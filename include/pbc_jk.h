@@ -133,8 +133,33 @@ int pbc_jk_overlap(const pbc_jk *h, double *S_host);
  */
 int pbc_jk_build(pbc_jk *h, const double *P, double *J, double *K, void *cuda_stream);
 
+/*
+ * Occupied-orbital entry point (the direction PAPER L941 names as future work for the reciprocal-space
+ * part): C is N x nocc fp64 row-major (DEVICE), the density is P = C C^T (eq 72, occupations folded into C).
+ * Same outputs and contract as pbc_jk_build; the reciprocal-space K contraction uses C itself as the factor of P
+ * (cost 8 nocc N^2 per G vector) instead of decomposing P.
+ */
+int pbc_jk_build_orbitals(pbc_jk *h, const double *C, int32_t nocc, double *J, double *K, void *cuda_stream);
+
 /* Same with HOST buffers: copies P host->device, builds, copies J/K back, synchronises. */
 int pbc_jk_build_host(pbc_jk *h, const double *P_host, double *J_host, double *K_host);
+
+/*
+ * One-electron Ewald terms of the same geometry.  Any output may be NULL.
+ *   T  (DEVICE, N x N, overwritten): kinetic matrix, SI eq S1 (L1151-1169; -1/2 Laplacian on the second function,
+ *      image-summed like the overlap).
+ *   V  (DEVICE, N x N, overwritten): V_mn = sum_C q_C (mn | point charge at atom C) under the zero-mean periodic
+ *      Coulomb kernel, Ewald-split as eq 52 (L372-386): erfc part over lattice images, reciprocal part through
+ *      rho_mn(G), and the -pi/(Omega w^2) S_mn sum_C q_C term.  Sign as in the paper: the electron-nucleus
+ *      attraction matrix is -V with q_C = Z_C.
+ *   e_nuc_host (HOST, one double): Ewald energy of the point charges, eq 91 (L679-686), including the
+ *      -pi/(Omega w^2) (sum q)^2 / 2 term of a charged cell.
+ * charges_host: natom doubles (HOST), one charge per atom of pbc_jk_create.  Enqueues on `cuda_stream` and
+ * synchronises it before returning (setup-time call, not part of the per-iteration build); uses the handle's
+ * build workspaces, so no build may be in flight.
+ */
+int pbc_jk_one_electron(pbc_jk *h, const double *charges_host, double *T, double *V, double *e_nuc_host,
+                        void *cuda_stream);
 
 /* `parts` bit 0 SR, bit 1 LR, bit 2 SELF (default 7): restrict the next builds to these terms of
  * eq 56 (bring-up and tests: the oracle returns the same parts separately). */

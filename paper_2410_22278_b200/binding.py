@@ -19,8 +19,8 @@ PBC_JK_OK = 0
 STATUS = {0: "OK", -1: "INVALID_ARG", -2: "NOMEM", -3: "CUDA", -4: "UNSUPPORTED"}
 
 # every symbol include/pbc_jk.h declares (checked by tests/test_abi.py)
-SYMBOLS = ["pbc_jk_create", "pbc_jk_nbf", "pbc_jk_overlap", "pbc_jk_build", "pbc_jk_build_host",
-           "pbc_jk_set_parts", "pbc_jk_set_shard", "pbc_jk_get_stats", "pbc_jk_set_profile", "pbc_jk_get_class_stats",
+SYMBOLS = ["pbc_jk_create", "pbc_jk_nbf", "pbc_jk_overlap", "pbc_jk_build", "pbc_jk_build_orbitals", "pbc_jk_build_host",
+           "pbc_jk_one_electron", "pbc_jk_set_parts", "pbc_jk_set_shard", "pbc_jk_get_stats", "pbc_jk_set_profile", "pbc_jk_get_class_stats",
            "pbc_jk_last_error", "pbc_jk_destroy"]
 
 
@@ -79,6 +79,8 @@ def load() -> C.CDLL:
         lib.pbc_jk_overlap.restype = C.c_int
         lib.pbc_jk_build.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         lib.pbc_jk_build.restype = C.c_int
+        lib.pbc_jk_build_orbitals.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p]
+        lib.pbc_jk_build_orbitals.restype = C.c_int
         lib.pbc_jk_build_host.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         lib.pbc_jk_build_host.restype = C.c_int
         lib.pbc_jk_set_parts.argtypes = [C.c_void_p, C.c_int32]
@@ -94,6 +96,8 @@ def load() -> C.CDLL:
         lib.pbc_jk_last_error.restype = C.c_char_p
         lib.pbc_jk_destroy.argtypes = [C.c_void_p]
         lib.pbc_jk_destroy.restype = C.c_int
+        lib.pbc_jk_one_electron.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.POINTER(C.c_double), C.c_void_p]
+        lib.pbc_jk_one_electron.restype = C.c_int
         lib.pbc_jk_set_shard.argtypes = [C.c_void_p, C.c_int32, C.c_int32]
         lib.pbc_jk_set_shard.restype = C.c_int
         _lib = lib
@@ -193,6 +197,23 @@ class PbcJK:
             m |= _PARTS[p.strip()]
         self._check(load().pbc_jk_set_parts(self._h, m))
 
+    def one_electron(self, charges, T=None, V=None, want_e_nuc: bool = True, stream=None):
+        """Kinetic matrix T, point-charge interaction matrix V (device tensors, overwritten) and the Ewald energy of the
+        charges (returned; None unless want_e_nuc).  charges: one per atom (host)."""
+        import torch
+
+        n = self.nbf
+        for t in (T, V):
+            if t is not None and not (t.is_cuda and t.dtype == torch.float64 and t.is_contiguous() and tuple(t.shape) == (n, n)):
+                raise ValueError("T, V must be contiguous float64 CUDA tensors of shape (nbf, nbf)")
+        q = np.ascontiguousarray(charges, dtype=np.float64)
+        assert q.shape == (self._keep["xyz"].shape[0],)
+        e = C.c_double()
+        st = torch.cuda.current_stream().cuda_stream if stream is None else int(stream)
+        self._check(load().pbc_jk_one_electron(self._h, q.ctypes.data, T.data_ptr() if T is not None else None,
+                                               V.data_ptr() if V is not None else None, C.byref(e) if want_e_nuc else None, st))
+        return float(e.value) if want_e_nuc else None
+
     def set_shard(self, rank: int = 0, nranks: int = 1):
         """This handle builds share `rank` of `nranks` of every J and K; the sum over ranks is the full matrix."""
         self._check(load().pbc_jk_set_shard(self._h, int(rank), int(nranks)))
@@ -219,6 +240,20 @@ class PbcJK:
         st = torch.cuda.current_stream().cuda_stream if stream is None else int(stream)
         self._check(load().pbc_jk_build(self._h, P.data_ptr(), J.data_ptr() if J is not None else None,
                                         K.data_ptr() if K is not None else None, st))
+
+    def build_orbitals(self, Corb, J=None, K=None, stream=None):
+        """Occupied-orbital entry point: Corb is a contiguous float64 CUDA tensor (nbf, nocc), P = Corb Corb^T."""
+        import torch
+
+        n = self.nbf
+        if not (Corb.is_cuda and Corb.dtype == torch.float64 and Corb.is_contiguous() and Corb.dim() == 2 and Corb.shape[0] == n):
+            raise ValueError("Corb must be a contiguous float64 CUDA tensor of shape (nbf, nocc)")
+        for t in (J, K):
+            if t is not None and not (t.is_cuda and t.dtype == torch.float64 and t.is_contiguous() and tuple(t.shape) == (n, n)):
+                raise ValueError("J, K must be contiguous float64 CUDA tensors of shape (nbf, nbf)")
+        st = torch.cuda.current_stream().cuda_stream if stream is None else int(stream)
+        self._check(load().pbc_jk_build_orbitals(self._h, Corb.data_ptr(), int(Corb.shape[1]), J.data_ptr() if J is not None else None,
+                                                 K.data_ptr() if K is not None else None, st))
 
     def build_host(self, P: np.ndarray, want_j: bool = True, want_k: bool = True):
         """Host numpy in, host numpy out (copies inside the library); synchronous."""

@@ -28,14 +28,16 @@ NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", 
 # headers each source includes (directly or not): a change recompiles only the units that see it
 _SR_H = ["pbcjk_common.h", "pbcjk_md.cuh", "pbcjk_sr.cuh"]
 _SRK_H = _SR_H + ["pbcjk_srk.cuh", "gen_sr_k.py"]     # the K evaluators are generated into csrc/build/gen
-HEADERS = {"pbcjk_api.cu": _SR_H + ["pbcjk_lr.cuh", os.path.join(INCLUDE, "pbc_jk.h")],
+HEADERS = {"pbcjk_api.cu": _SR_H + ["pbcjk_lr.cuh", "pbcjk_1e.cuh", os.path.join(INCLUDE, "pbc_jk.h")],
            "pbcjk_lr.cu": ["pbcjk_common.h", "pbcjk_md.cuh", "pbcjk_lr.cuh"],
+           "pbcjk_1e.cu": _SR_H + ["pbcjk_lr.cuh", "pbcjk_1e.cuh"],
            "sr_dispatch.cu": _SR_H, "sr_j_inst.cu": _SR_H, "sr_k_inst.cu": _SRK_H, "bench_peaks.cu": []}
 
 
 def _units():
     """(object name, source, extra defines)"""
-    u = [("api", "pbcjk_api.cu", []), ("lr", "pbcjk_lr.cu", []), ("sr_dispatch", "sr_dispatch.cu", [])]
+    u = [("api", "pbcjk_api.cu", []), ("lr", "pbcjk_lr.cu", []), ("one_electron", "pbcjk_1e.cu", []),
+         ("sr_dispatch", "sr_dispatch.cu", [])]
     for lb in range(5):
         u.append((f"sr_j_{lb}", "sr_j_inst.cu", [f"-DJ_LB={lb}"]))
     for la in range(3):

@@ -2,6 +2,7 @@
 // orchestration (A4-A10).  All arithmetic of the path runs in the CUDA kernels of this directory.
 #include "../../include/pbc_jk.h"
 #include "pbcjk_common.h"
+#include "pbcjk_1e.cuh"
 #include "pbcjk_lr.cuh"
 #include "pbcjk_sr.cuh"
 
@@ -51,7 +52,7 @@ struct DevPool {
 
 struct HostPair {
     int shA, shB;
-    double p, ip, P[3], PA[3], PB[3], coef, lb;
+    double p, ip, P[3], PA[3], PB[3], coef, lb, b;
 };
 
 }  // namespace
@@ -109,6 +110,8 @@ struct pbc_jk {
     int64_t n_prim_pairs = 0, n_sp_images = 0;
     double create_seconds = 0.0;
     std::vector<double> S_host;
+    std::vector<double> atom_xyz;        // atom positions folded into the home cell (host copy; one-electron terms)
+    double omega = 0.0;
 };
 
 namespace {
@@ -226,7 +229,7 @@ int setup(pbc_jk *h, const pbc_cell *cell, const pbc_atoms *atoms, const pbc_she
 
     // ---- basis bookkeeping ----
     const int ns = shells->nshell, natom = atoms->natom;
-    h->nshell = ns; h->natom = natom;
+    h->nshell = ns; h->natom = natom; h->omega = omega;
     // every centre may be given in any lattice image (L781): fold all of them into the home cell, so that the
     // lattice indices the real-space scans enumerate stay inside the packed 10-bit range checked below
     std::vector<double> axyz(3 * (size_t)natom);
@@ -236,6 +239,7 @@ int setup(pbc_jk *h, const pbc_cell *cell, const pbc_atoms *atoms, const pbc_she
         for (int k = 0; k < 3; ++k) f[k] = std::floor(lat.binv[3 * k] * r[0] + lat.binv[3 * k + 1] * r[1] + lat.binv[3 * k + 2] * r[2]);
         for (int x = 0; x < 3; ++x) axyz[3 * a + x] = r[x] - (f[0] * lat.a[x] + f[1] * lat.a[3 + x] + f[2] * lat.a[6 + x]);
     }
+    h->atom_xyz = axyz;
     std::vector<int> sh_l(ns), sh_ao(ns), sh_atom(ns);
     std::vector<double> scx(ns), scy(ns), scz(ns);
     int nbf = 0, nprim_tot = 0;
@@ -350,7 +354,7 @@ int setup(pbc_jk *h, const pbc_cell *cell, const pbc_atoms *atoms, const pbc_she
                     const double bound = q.cc * ang * ex;
                     if (!(bound > d_pair)) continue;
                     HostPair e;
-                    e.shA = A; e.shB = B; e.p = q.p; e.ip = 1.0 / q.p;
+                    e.shA = A; e.shB = B; e.p = q.p; e.ip = 1.0 / q.p; e.b = q.b;
                     for (int x = 0; x < 3; ++x) {
                         e.P[x] = (q.a * RA[x] + q.b * Bt[x]) / q.p;
                         e.PA[x] = e.P[x] - RA[x];
@@ -554,6 +558,11 @@ int setup(pbc_jk *h, const pbc_cell *cell, const pbc_atoms *atoms, const pbc_she
         CK(pool.upload(&U.coef, soa(up, 3, 0))); CK(pool.upload(&U.lb, soa(up, 4, 0)));
         CK(pool.upload(&U.PAx, soa(up, 5, 0))); CK(pool.upload(&U.PAy, soa(up, 5, 1))); CK(pool.upload(&U.PAz, soa(up, 5, 2)));
         CK(pool.upload(&U.PBx, soa(up, 6, 0))); CK(pool.upload(&U.PBy, soa(up, 6, 1))); CK(pool.upload(&U.PBz, soa(up, 6, 2)));
+        {
+            std::vector<double> bexp(up.size());
+            for (size_t i = 0; i < up.size(); ++i) bexp[i] = up[i].b;
+            CK(pool.upload(&U.bexp, bexp));
+        }
         CK(pool.upload(&U.sp, u_sp)); CK(pool.upload(&U.sp_off, sp_off));
         CK(pool.upload(&U.sp_shA, sp_shA)); CK(pool.upload(&U.sp_shB, sp_shB));
         // shell pairs by class (l_A, l_B): one rho_mn(G) kernel instantiation per class
@@ -836,10 +845,25 @@ int pbc_jk_set_shard(pbc_jk *h, int32_t rank, int32_t nranks)
     return PBC_JK_OK;
 }
 
+static int build_impl(pbc_jk *h, const double *P, const double *Corb, int nocc, double *J, double *K, void *cuda_stream);
+
 int pbc_jk_build(pbc_jk *h, const double *P, double *J, double *K, void *cuda_stream)
 {
     if (!h) return PBC_JK_ERR_INVALID_ARG;
     if (!P) return fail(h, PBC_JK_ERR_INVALID_ARG, "P is null");
+    return build_impl(h, P, nullptr, 0, J, K, cuda_stream);
+}
+
+int pbc_jk_build_orbitals(pbc_jk *h, const double *C, int32_t nocc, double *J, double *K, void *cuda_stream)
+{
+    if (!h) return PBC_JK_ERR_INVALID_ARG;
+    if (!C) return fail(h, PBC_JK_ERR_INVALID_ARG, "C is null");
+    if (nocc < 1 || nocc > h->N) return fail(h, PBC_JK_ERR_INVALID_ARG, "nocc must be in 1..N");
+    return build_impl(h, nullptr, C, nocc, J, K, cuda_stream);
+}
+
+static int build_impl(pbc_jk *h, const double *P, const double *Corb, int nocc, double *J, double *K, void *cuda_stream)
+{
     {
         int dev = -1;
         CK(cudaGetDevice(&dev));
@@ -850,6 +874,10 @@ int pbc_jk_build(pbc_jk *h, const double *P, double *J, double *K, void *cuda_st
     const size_t NN = (size_t)N * N;
     const bool doSR = h->parts & 1, doLR = h->parts & 2, doSELF = (h->parts & 4) && h->shard_rank == 0;
     const bool prof = h->profile;
+    if (Corb) {                          // P = C C^T into the staging buffer of build_host (not in use by this entry point)
+        launch_density_from_orbitals(Corb, N, nocc, h->hostP, st);
+        P = h->hostP;
+    }
     CK(cudaMemsetAsync(h->counters, 0, CNT_N * 8, st));
     CK(cudaEventRecord(h->ev[0], st));
     int64_t nl = 0;                      // kernels launched by this build
@@ -858,7 +886,7 @@ int pbc_jk_build(pbc_jk *h, const double *P, double *J, double *K, void *cuda_st
     // ---- A4: density prep ----
     launch_scale_density(P, h->Pp, h->mixed ? h->Ppf : nullptr, N, Np, h->fcomp, h->maxbits, h->lnPmax, h->counters + CNT_FLAG, st);
     launch_density_blocks(h->Pp, Np, h->sh, h->KJ, h->lnPblk, h->lnProw, h->kjP, st);
-    nl += 4 + (h->KJ.n > 0);
+    nl += 4 + (h->KJ.n > 0) + (Corb ? 1 : 0);
     SRParams sp;
     sp.K = h->K; sp.U = h->U; sp.KJ = h->KJ; sp.lat = h->lat; sp.sh = h->sh;
     sp.boys = h->boys; sp.Pp = h->Pp; sp.Ppf = h->Ppf; sp.ldP = Np; sp.Dt = h->Dt; sp.Jt = h->Jt; sp.Ksr = h->Ksr;
@@ -938,8 +966,13 @@ int pbc_jk_build(pbc_jk *h, const double *P, double *J, double *K, void *cuda_st
     const size_t strideK = (size_t)Np * Np;
     // K^LR = sum_slots Y^T Y with Y = L^T A', P' = L L^T (device-side rank; dense fallback inside the same kernels)
     if (needKlr) {
-        launch_factor_density(h->Pp, N, Np, h->LT, h->chol_d, h->chol_dyn, h->chol_s, h->Zstack, st);
-        nl += factor_density_launches(N);
+        if (Corb) {                      // the orbitals are the factor: no decomposition
+            launch_factor_from_orbitals(Corb, N, nocc, Np, h->fcomp, h->LT, h->chol_dyn, st);
+            nl += 1;
+        } else {
+            launch_factor_density(h->Pp, N, Np, h->LT, h->chol_d, h->chol_dyn, h->chol_s, h->Zstack, st);
+            nl += factor_density_launches(N);
+        }
     }
     // one batch of S slots (layout A'[row*Np*S + col*S + slot]):  Y = L^T A'  (rows >= rank skipped), then
     // K += alpha sum_r sum_slot Y[r][mu][slot] Y[r][nu][slot] on the lower tiles (batches = rows r of the factor)
@@ -1011,6 +1044,116 @@ int pbc_jk_build(pbc_jk *h, const double *P, double *J, double *K, void *cuda_st
     h->last_stream = st;
     h->built = true;
     h->profiled_last = prof;
+    return PBC_JK_OK;
+}
+
+// Ewald energy of the point charges (eq 91) on the host: O(natom^2 images + natom N_G), once per geometry.
+static double ewald_point_charges(const pbc_jk *h, const double *q)
+{
+    const Lattice &lat = h->lat;
+    const int na = h->natom;
+    const double w = h->omega, w2 = w * w;
+    const double *x = h->atom_xyz.data();
+    const double delta = 1e-18;
+    double qtot = 0.0, q2 = 0.0;
+    for (int a = 0; a < na; ++a) { qtot += q[a]; q2 += q[a] * q[a]; }
+    // real space: erfc(w r)/r < e^{-w^2 r^2} below delta (eq 92-93)
+    const double rb = std::sqrt(std::log(1.0 / delta)) / w;
+    double e_sr = 0.0;
+#pragma omp parallel for reduction(+ : e_sr) schedule(dynamic, 4)
+    for (int a = 0; a < na; ++a)
+        for (int b = a; b < na; ++b) {
+            if (q[a] == 0.0 || q[b] == 0.0) continue;
+            const double d[3] = {x[3 * a] - x[3 * b], x[3 * a + 1] - x[3 * b + 1], x[3 * a + 2] - x[3 * b + 2]};
+            const double md[3] = {-d[0], -d[1], -d[2]};
+            double sum = 0.0;
+            for_images_host(lat, md, rb, [&](const double *T) {
+                const double v0 = d[0] + T[0], v1 = d[1] + T[1], v2 = d[2] + T[2];
+                const double r = std::sqrt(v0 * v0 + v1 * v1 + v2 * v2);
+                if (r > 1e-12) sum += std::erfc(w * r) / r;
+            });
+            e_sr += (a == b ? 0.5 : 1.0) * q[a] * q[b] * sum;
+        }
+    // reciprocal space: full sphere, 4 pi/(Omega G^2) e^{-G^2/4w^2} |sum q e^{-iG.C}|^2 / 2 (cutoff eq 94 at delta)
+    const double gcut = 2.0 * w * std::sqrt(std::log(1.0 / delta));
+    int mmax[3];
+    for (int k = 0; k < 3; ++k) {
+        const double an = std::sqrt(lat.a[3 * k] * lat.a[3 * k] + lat.a[3 * k + 1] * lat.a[3 * k + 1] + lat.a[3 * k + 2] * lat.a[3 * k + 2]);
+        mmax[k] = (int)std::ceil(gcut * an / (2.0 * M_PI));
+    }
+    double e_lr = 0.0;
+#pragma omp parallel for reduction(+ : e_lr) schedule(dynamic, 1)
+    for (int m0 = -mmax[0]; m0 <= mmax[0]; ++m0)
+        for (int m1 = -mmax[1]; m1 <= mmax[1]; ++m1)
+            for (int m2 = -mmax[2]; m2 <= mmax[2]; ++m2) {
+                if (m0 == 0 && m1 == 0 && m2 == 0) continue;
+                double G[3];
+                for (int k = 0; k < 3; ++k) G[k] = 2.0 * M_PI * (m0 * lat.binv[k] + m1 * lat.binv[3 + k] + m2 * lat.binv[6 + k]);
+                const double G2 = G[0] * G[0] + G[1] * G[1] + G[2] * G[2];
+                if (G2 >= gcut * gcut) continue;
+                double nr = 0.0, ni = 0.0;
+                for (int a = 0; a < na; ++a) {
+                    const double ph = -(G[0] * x[3 * a] + G[1] * x[3 * a + 1] + G[2] * x[3 * a + 2]);
+                    nr += q[a] * std::cos(ph); ni += q[a] * std::sin(ph);
+                }
+                e_lr += 0.5 * 4.0 * M_PI / (lat.volume * G2) * std::exp(-G2 / (4.0 * w2)) * (nr * nr + ni * ni);
+            }
+    const double e_c = -M_PI / (lat.volume * w2) * 0.5 * qtot * qtot - w / std::sqrt(M_PI) * q2;
+    return e_sr + e_lr + e_c;
+}
+
+int pbc_jk_one_electron(pbc_jk *h, const double *charges_host, double *T, double *V, double *e_nuc_host, void *cuda_stream)
+{
+    if (!h) return PBC_JK_ERR_INVALID_ARG;
+    if ((V || e_nuc_host) && !charges_host) return fail(h, PBC_JK_ERR_INVALID_ARG, "charges are null");
+    {
+        int dev = -1;
+        CK(cudaGetDevice(&dev));
+        if (dev != h->device) return fail(h, PBC_JK_ERR_INVALID_ARG, "the handle was created on another CUDA device than the current one");
+    }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const int N = h->N, Np = h->Np, na = h->natom;
+    if (T) launch_kinetic(h->U, h->sh, h->fcomp, T, N, st);
+    if (V) {
+        // device copies of the charges and the folded atom positions (not on the per-iteration path: allocated here)
+        double *dq = nullptr, *dx = nullptr;
+        CK(cudaMalloc(&dq, sizeof(double) * na));
+        if (cudaMalloc(&dx, sizeof(double) * 3 * na) != cudaSuccess) { cudaFree(dq); return fail(h, PBC_JK_ERR_NOMEM, "device allocation failed"); }
+        cudaMemcpyAsync(dq, charges_host, sizeof(double) * na, cudaMemcpyHostToDevice, st);
+        cudaMemcpyAsync(dx, h->atom_xyz.data(), sizeof(double) * 3 * na, cudaMemcpyHostToDevice, st);
+        double qmax = 0.0;
+        for (int a = 0; a < na; ++a) qmax = std::max(qmax, std::fabs(charges_host[a]));
+        const size_t NN = (size_t)N * N;
+        // short range: Hermite-basis Vt of every pair-image (workspace Jt), back-transformed into Jsr (eq 96-97)
+        cudaMemsetAsync(h->Jt, 0, (size_t)nherm(4) * std::max(h->U.n, 1) * 8, st);
+        cudaMemsetAsync(h->Jsr, 0, NN * 8, st);
+        cudaMemsetAsync(h->Jlr, 0, NN * 8, st);
+        const double d_pair = h->cut.d_pair > 0 ? h->cut.d_pair : 1e-14;
+        launch_sr_v(h->U, h->lat, h->boys, h->jbra, h->njbra, dx, dq, na, qmax, std::log(d_pair * 1e-2), h->KJ.g0, h->KJ.rc, h->Jt, st);
+        if (h->U.nsp > 0) launch_j_backtransform(h->U, h->sh, h->Jt, h->Jsr, N, st);
+        // long range: J^LR with rho(G) replaced by the structure factor of the charges; SELF: the G = 0 slot
+        auto set_layout = [&](int S) {
+            if (h->cur_S == S) return;
+            h->cur_S = S;
+            cudaMemsetAsync(h->Astack, 0, (size_t)Np * Np * S * sizeof(double), st);
+        };
+        for (int g0 = 0; g0 < h->nG; g0 += h->nb) {
+            const int nb = std::min(h->nb, h->nG - g0), S = ((2 * nb + 15) / 16) * 16;
+            set_layout(S);
+            launch_agen(h->lr, g0, nb, S, 0.0, h->Astack, st);
+            launch_rho_nuc(h->lr, g0, nb, S, 0.0, dx, dq, na, h->rho, st);
+            launch_jlr_accum(h->Astack, Np, N, S, h->rho, 1.0, h->Jlr, st);
+        }
+        set_layout(16);
+        launch_agen(h->lr, -1, 1, 16, std::sqrt(h->c0), h->Astack, st);
+        launch_rho_nuc(h->lr, -1, 1, 16, std::sqrt(h->c0), dx, dq, na, h->rho, st);
+        launch_jlr_accum(h->Astack, Np, N, 16, h->rho, -1.0, h->Jlr, st);
+        launch_finalize_j(h->Jsr, h->Jlr, N, h->fcomp, V, st);
+        CK(cudaStreamSynchronize(st));
+        cudaFree(dq); cudaFree(dx);
+    }
+    if (e_nuc_host) *e_nuc_host = ewald_point_charges(h, charges_host);
+    CK(cudaGetLastError());
     return PBC_JK_OK;
 }
 

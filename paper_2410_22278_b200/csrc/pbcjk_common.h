@@ -55,6 +55,7 @@ struct PairListU {
     int n, nsp;
     const double *Px, *Py, *Pz, *p, *ip, *coef, *lb;
     const double *PAx, *PAy, *PAz, *PBx, *PBy, *PBz;
+    const double *bexp;                              // exponent b of the second (translated) primitive (kinetic integral)
     const int *sp;                                   // shell-pair index of each entry
     const int *sp_off;                               // [nsp + 1]
     const int *sp_shA, *sp_shB;                      // [nsp]

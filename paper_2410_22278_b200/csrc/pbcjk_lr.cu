@@ -693,6 +693,39 @@ __global__ void chol_fallback_kernel(const double *__restrict__ Pp, int N, int N
     if (idx == 0) { dyn[0] = N; dyn[1] = 1; }
 }
 
+// Occupied-orbital entry point: the caller hands C (N x nocc, row-major) with P = C C^T.
+//   P[m][n] = sum_i C[m][i] C[n][i]                                        (eq 72 L547 with the occupation folded into C)
+//   LT[i][m] = f_m C[m][i], rank = nocc: the factor P' = L L^T of the K^LR contraction without a decomposition
+__global__ void density_from_orbitals_kernel(const double *__restrict__ C, int N, int nocc, double *__restrict__ P)
+{
+    const int n = blockIdx.x * blockDim.x + threadIdx.x, m = blockIdx.y;
+    if (n >= N) return;
+    const double *cm = C + (size_t)m * nocc, *cn = C + (size_t)n * nocc;
+    double a0 = 0.0, a1 = 0.0;
+    int i = 0;
+    for (; i + 2 <= nocc; i += 2) { a0 = fma(cm[i], cn[i], a0); a1 = fma(cm[i + 1], cn[i + 1], a1); }
+    if (i < nocc) a0 = fma(cm[i], cn[i], a0);
+    P[(size_t)m * N + n] = a0 + a1;
+}
+__global__ void factor_from_orbitals_kernel(const double *__restrict__ C, int N, int nocc, int Np, const double *__restrict__ f,
+                                            double *__restrict__ LT, int *dyn)
+{
+    const int m = blockIdx.x * blockDim.x + threadIdx.x, i = blockIdx.y;
+    if (m < N) LT[(size_t)i * Np + m] = f[m] * C[(size_t)m * nocc + i];
+    if (m == 0 && i == 0) { dyn[0] = nocc; dyn[1] = 0; dyn[2] = 1; }
+}
+void launch_density_from_orbitals(const double *C, int N, int nocc, double *P, cudaStream_t st)
+{
+    dim3 grid((N + 127) / 128, N);
+    density_from_orbitals_kernel<<<grid, 128, 0, st>>>(C, N, nocc, P);
+}
+void launch_factor_from_orbitals(const double *C, int N, int nocc, int Np, const double *fcomp, double *LT, int *dyn, cudaStream_t st)
+{
+    cudaMemsetAsync(LT, 0, (size_t)Np * Np * sizeof(double), st);
+    dim3 grid((N + 127) / 128, nocc);
+    factor_from_orbitals_kernel<<<grid, 128, 0, st>>>(C, N, nocc, Np, fcomp, LT, dyn);
+}
+
 void launch_factor_density(const double *Pp, int N, int Np, double *LT, double *dbuf, int *dyn, double *dscal, double *scratch,
                            cudaStream_t st)
 {

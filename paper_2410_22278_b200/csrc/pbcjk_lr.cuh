@@ -65,6 +65,9 @@ void launch_dgemm(const GemmArgs &g, cudaStream_t st);
 void launch_factor_density(const double *Pp, int N, int Np, double *LT, double *dbuf, int *dyn, double *dscal, double *scratch,
                            cudaStream_t st);
 int factor_density_launches(int N);
+// occupied-orbital entry point: P = C C^T (N x N, unscaled) and the factor LT = (f C)^T with rank nocc (dyn as above)
+void launch_density_from_orbitals(const double *C, int N, int nocc, double *P, cudaStream_t st);
+void launch_factor_from_orbitals(const double *C, int N, int nocc, int Np, const double *fcomp, double *LT, int *dyn, cudaStream_t st);
 // out = f f (sum of parts), symmetrised; see pbcjk_lr.cu
 void launch_finalize_j(const double *Jsr, const double *Jlr, int N, const double *fcomp, double *J, cudaStream_t st);
 void launch_finalize_k(const double *Ksr, const ShellInfo &sh, const double *Klr, int nsplit, size_t strideK, int Np,

@@ -63,18 +63,23 @@ class Workload:
         return rng.standard_normal((self.nbf, self.n_occ))
 
 
+def orthonormal_orbitals(C0: np.ndarray, S: np.ndarray) -> np.ndarray:
+    """C = C0 (C0^T S C0)^(-1/2): seeded orbitals orthonormalised under the overlap matrix (SURVEY C-19)."""
+    M = C0.T @ S @ C0
+    M = 0.5 * (M + M.T)
+    w, V = np.linalg.eigh(M)
+    if w.min() <= 0:
+        raise ValueError("C0^T S C0 is not positive definite")
+    return C0 @ (V * (1.0 / np.sqrt(w))) @ V.T
+
+
 def density_from_orbitals(C0: np.ndarray, S: np.ndarray) -> np.ndarray:
     """P = C C^T with C = C0 (C0^T S C0)^(-1/2)  (SURVEY C-19, tr(PS) = n_occ).
 
     Plain linear algebra on inputs; S comes from the caller (oracle S in the
     tests, the library's own S in bench.py).
     """
-    M = C0.T @ S @ C0
-    M = 0.5 * (M + M.T)
-    w, V = np.linalg.eigh(M)
-    if w.min() <= 0:
-        raise ValueError("C0^T S C0 is not positive definite")
-    C = C0 @ (V * (1.0 / np.sqrt(w))) @ V.T
+    C = orthonormal_orbitals(C0, S)
     P = C @ C.T
     return 0.5 * (P + P.T)
 

@@ -278,3 +278,60 @@ def test_mixed_precision_full_matrices(torch_cuda, oracle_mod, name):
     dK2 = np.abs(K2 - ref["K"]).max()
     print(f"  all-fp32 quartets: max|dK| = {dK2:.3e}")
     assert dK2 < 1e-4 * max(1.0, np.abs(ref["K"]).max())
+
+
+@pytest.mark.parametrize("name", ["tiny", "pd_test", "water8"])
+def test_one_electron_terms(torch_cuda, oracle_mod, name):
+    """kinetic matrix (SI eq S1), point-charge interaction matrix V (eq 52) and the Ewald energy of the
+    charges (eq 91) against the oracle; a charged set of point charges on purpose (the -pi/(Omega w^2) terms matter)."""
+    from paper_2410_22278_b200 import workloads
+    from paper_2410_22278_b200.binding import PbcJK
+    torch = torch_cuda
+    wl = workloads.get(name)
+    rng = np.random.default_rng(17)
+    q = rng.uniform(0.5, 8.0, wl.natom) * rng.choice([1.0, 1.0, -1.0], wl.natom)
+    ref = oracle_mod.one_electron(wl, q)
+    with PbcJK(wl) as h:
+        T = torch.empty((wl.nbf, wl.nbf), dtype=torch.float64, device="cuda")
+        V = torch.empty_like(T)
+        e = h.one_electron(q, T, V)
+        torch.cuda.synchronize()
+        # the J/K build still works afterwards (shared workspaces)
+        P, _ = _density(oracle_mod, wl)
+        Pd = torch.from_numpy(P).cuda()
+        J = torch.empty_like(Pd)
+        h.build(Pd, J, None)
+        torch.cuda.synchronize()
+        e2 = h.one_electron(q, None, None)
+    T, V = T.cpu().numpy(), V.cpu().numpy()
+    scale = max(1.0, np.abs(q).max())
+    assert np.abs(T - ref["T"]).max() < 1e-10
+    assert np.abs(V - ref["V"]).max() < TOL * scale, np.abs(V - ref["V"]).max()
+    assert abs(e - ref["E_nuc"]) < 1e-9 * max(1.0, abs(ref["E_nuc"])) and abs(e2 - e) < 1e-11
+    assert np.abs(T - T.T).max() < 1e-12 and np.abs(V - V.T).max() < 1e-11
+    if name == "tiny":
+        Jref = oracle_mod.jk(wl, P, which="j")["J"]
+        assert np.abs(J.cpu().numpy() - Jref).max() < TOL
+
+
+@pytest.mark.parametrize("name", ["pd_test", "water8"])
+def test_orbital_entry_point(torch_cuda, oracle_mod, name):
+    """pbc_jk_build_orbitals: handing C with P = C C^T gives the oracle's J and K of that P, and the same
+    matrices as pbc_jk_build (which factors P itself) to rounding."""
+    from paper_2410_22278_b200 import workloads
+    from paper_2410_22278_b200.binding import PbcJK
+    torch = torch_cuda
+    wl = workloads.get(name)
+    S = oracle_mod.overlap(wl)
+    Cn = workloads.orthonormal_orbitals(wl.orbitals_seed(), S)
+    P = Cn @ Cn.T
+    ref = oracle_mod.jk(wl, 0.5 * (P + P.T))
+    with PbcJK(wl) as h:
+        Cd = torch.from_numpy(np.ascontiguousarray(Cn)).cuda()
+        J, K, J2, K2 = (torch.empty((wl.nbf, wl.nbf), dtype=torch.float64, device="cuda") for _ in range(4))
+        h.build_orbitals(Cd, J, K)
+        h.build(torch.from_numpy(0.5 * (P + P.T)).cuda(), J2, K2)
+        torch.cuda.synchronize()
+        assert h.stats()["rank_p"] == wl.n_occ
+    assert np.abs(J.cpu().numpy() - ref["J"]).max() < TOL and np.abs(K.cpu().numpy() - ref["K"]).max() < TOL
+    assert (J - J2).abs().max().item() < 1e-11 and (K - K2).abs().max().item() < 1e-11
