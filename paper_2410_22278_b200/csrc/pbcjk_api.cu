@@ -738,9 +738,9 @@ int setup(pbc_jk *h, const pbc_cell *cell, const pbc_atoms *atoms, const pbc_she
         CK(pool.alloc(&h->Klr, (size_t)h->nsplit * Np * Np));
         CK(pool.alloc(&h->Astack, Np * h->ld)); CK(cudaMemset(h->Astack, 0, Np * h->ld * 8));
         CK(pool.alloc(&h->Zstack, Np * h->ld));
-        CK(pool.alloc(&h->rho, (size_t)rho_scratch_doubles(h->Smax, nbf)));
+        CK(pool.alloc(&h->rho, (size_t)rho_scratch_doubles(h->Smax, agen_groups_total(h->lr))));
         CK(pool.alloc(&h->LT, Np * Np)); CK(pool.alloc(&h->chol_d, 2 * Np)); CK(pool.alloc(&h->chol_s, 2));
-        CK(pool.alloc(&h->chol_dyn, 4));
+        CK(pool.alloc(&h->chol_dyn, 8));      // rank, fallback flag, done, -, grid barrier (2)
         CK(pool.alloc(&h->hostP, N * N)); CK(pool.alloc(&h->hostJ, N * N)); CK(pool.alloc(&h->hostK, N * N));
         for (auto &e : h->ev) CK(cudaEventCreate(&e));
         h->evG.assign(2 * ((size_t)(h->nG + h->nb - 1) / h->nb + 2), nullptr);
@@ -755,7 +755,7 @@ int setup(pbc_jk *h, const pbc_cell *cell, const pbc_atoms *atoms, const pbc_she
     // ---- A3: overlap S = rho_mn(G = 0) (eq 21) ----
     {
         h->cur_S = 16;                   // the whole stack was zero-filled at allocation
-        launch_agen(h->lr, -1, 1, 16, 1.0, h->Astack, 0);
+        launch_agen(h->lr, -1, 1, 16, 1.0, h->Astack, nullptr, nullptr, 0);
         double *dS = h->hostJ;
         launch_extract_overlap(h->Astack, h->Np, 16, nbf, h->fcomp, dS, 0);
         h->S_host.resize((size_t)nbf * nbf);
@@ -1007,10 +1007,10 @@ static int build_impl(pbc_jk *h, const double *P, const double *Corb, int nocc, 
             if (ibatch % h->shard_n != h->shard_rank) continue;      // multi-GPU: G batches dealt round-robin
             const int nb = std::min(h->nb, h->nG - g0), S = ((2 * nb + 15) / 16) * 16;
             CK(set_layout(S));
-            launch_agen(h->lr, g0, nb, S, 0.0, h->Astack, st);
+            launch_agen(h->lr, g0, nb, S, 0.0, h->Astack, h->Pp, J ? h->rho : nullptr, st);
             nl += n_agen + (J ? 3 : 0) + (K ? 2 : 0);
             if (J) {
-                launch_rho_reduce(h->Pp, h->Astack, Np, N, S, h->rho, st);
+                launch_rho_final(h->lr, S, h->rho, st);
                 launch_jlr_accum(h->Astack, Np, N, S, h->rho, 1.0, h->Jlr, st);
             }
             if (K) klr_batch(S, 1.0, h->nsplit);
@@ -1019,10 +1019,10 @@ static int build_impl(pbc_jk *h, const double *P, const double *Corb, int nocc, 
     // ---- A9: the G = 0 slot, weight -pi/(Omega w^2), A = S ----
     if (doSELF) {
         CK(set_layout(16));
-        launch_agen(h->lr, -1, 1, 16, std::sqrt(h->c0), h->Astack, st);
+        launch_agen(h->lr, -1, 1, 16, std::sqrt(h->c0), h->Astack, h->Pp, J ? h->rho : nullptr, st);
         nl += n_agen + (J ? 3 : 0) + (K ? 2 : 0);
         if (J) {
-            launch_rho_reduce(h->Pp, h->Astack, Np, N, 16, h->rho, st);
+            launch_rho_final(h->lr, 16, h->rho, st);
             launch_jlr_accum(h->Astack, Np, N, 16, h->rho, -1.0, h->Jlr, st);
         }
         if (K) klr_batch(16, -1.0, h->nsplit);
@@ -1140,12 +1140,12 @@ int pbc_jk_one_electron(pbc_jk *h, const double *charges_host, double *T, double
         for (int g0 = 0; g0 < h->nG; g0 += h->nb) {
             const int nb = std::min(h->nb, h->nG - g0), S = ((2 * nb + 15) / 16) * 16;
             set_layout(S);
-            launch_agen(h->lr, g0, nb, S, 0.0, h->Astack, st);
+            launch_agen(h->lr, g0, nb, S, 0.0, h->Astack, nullptr, nullptr, st);
             launch_rho_nuc(h->lr, g0, nb, S, 0.0, dx, dq, na, h->rho, st);
             launch_jlr_accum(h->Astack, Np, N, S, h->rho, 1.0, h->Jlr, st);
         }
         set_layout(16);
-        launch_agen(h->lr, -1, 1, 16, std::sqrt(h->c0), h->Astack, st);
+        launch_agen(h->lr, -1, 1, 16, std::sqrt(h->c0), h->Astack, nullptr, nullptr, st);
         launch_rho_nuc(h->lr, -1, 1, 16, std::sqrt(h->c0), dx, dq, na, h->rho, st);
         launch_jlr_accum(h->Astack, Np, N, 16, h->rho, -1.0, h->Jlr, st);
         launch_finalize_j(h->Jsr, h->Jlr, N, h->fcomp, V, st);

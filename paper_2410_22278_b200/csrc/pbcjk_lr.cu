@@ -10,6 +10,7 @@
 // the FP64 tensor cores (DMMA, mma.sync.m8n8k4.f64) -- tcgen05 has no f64 kind.
 #include "pbcjk_lr.cuh"
 #include "pbcjk_md.cuh"
+#include <algorithm>
 #include <cmath>
 
 namespace pbcjk {
@@ -238,14 +239,22 @@ void launch_j_backtransform(const PairListU &U, const ShellInfo &sh, const doubl
 // (slot 2g = Re, 2g+1 = Im of G number g of the batch, weight sqrt(w) folded in; slots past the batch are 0).
 // One block per shell pair of class (LA, LB), threads over the G of the batch: each thread writes its (Re, Im)
 // pair as one 16-byte store, so a warp writes 512 contiguous bytes per matrix element.
+// A CTA takes AGEN_PAIRS consecutive shell pairs of its class; with `rho_part` it also forms its share of
+//   rho'[slot] = sum_mn P'_mn A'_mn[slot]      (eq 98 first term: the density's Fourier coefficients)
+// from the values it has in registers -- one partial per (CTA, slot), summed in a fixed order by rho_final_kernel -- so
+// the stored batch is not streamed a second time for it.
+constexpr int AGEN_PAIRS = 8;
 template <int LA, int LB>
-__global__ void __launch_bounds__(64) agen_kernel(LRParams p, const int *__restrict__ sp_list, int g0, int nb, int S, double w0,
-                                                  double *__restrict__ Astack, size_t ld)
+__global__ void __launch_bounds__(64) agen_kernel(LRParams p, const int *__restrict__ sp_list, int nsp_cls, int g0, int nb, int S,
+                                                  double w0, double *__restrict__ Astack, size_t ld, const double *__restrict__ Pp,
+                                                  double *__restrict__ rho_part)
 {
     constexpr int NA = ncart(LA), NB = ncart(LB);
-    const int sp = sp_list[blockIdx.x];
     const int gl = blockIdx.y * blockDim.x + threadIdx.x;
     if (2 * gl >= S) return;
+    double rr = 0.0, ri = 0.0;
+    for (int ip = blockIdx.x * AGEN_PAIRS; ip < min((blockIdx.x + 1) * AGEN_PAIRS, nsp_cls); ++ip) {
+    const int sp = sp_list[ip];
     const bool overlap = g0 < 0;
     const bool live = gl < nb;
     double Gx = 0, Gy = 0, Gz = 0, sw = live ? w0 : 0.0;
@@ -311,15 +320,33 @@ __global__ void __launch_bounds__(64) agen_kernel(LRParams p, const int *__restr
             const double2 v = make_double2(accr[a * NB + b], overlap ? 0.0 : acci[a * NB + b]);
             *reinterpret_cast<double2 *>(Astack + (size_t)(oa + a) * ld + (size_t)(ob + b) * S + 2 * gl) = v;
             *reinterpret_cast<double2 *>(Astack + (size_t)(ob + b) * ld + (size_t)(oa + a) * S + 2 * gl) = v;
+            if (rho_part) {
+                const double pv = (A != B ? 2.0 : 1.0) * Pp[(size_t)(oa + a) * p.Np + ob + b];     // (m,n) and (n,m)
+                rr = fma(pv, v.x, rr);
+                ri = fma(pv, v.y, ri);
+            }
         }
+    }
+    if (rho_part) *reinterpret_cast<double2 *>(rho_part + (size_t)blockIdx.x * S + 2 * gl) = make_double2(rr, ri);
+}
+static int agen_groups(const LRParams &p, int c) { return (p.n_sp_cls[c] + AGEN_PAIRS - 1) / AGEN_PAIRS; }
+int agen_groups_total(const LRParams &p)
+{
+    int n = 0;
+    for (int c = 0; c < 9; ++c) n += agen_groups(p, c);
+    return n;
 }
 template <int LA, int LB>
-static void launch_agen_class(const LRParams &p, int g0, int nb, int S, double w0, double *Astack, size_t ld, cudaStream_t st)
+static void launch_agen_class(const LRParams &p, int g0, int nb, int S, double w0, double *Astack, size_t ld, const double *Pp,
+                              double *rho_part, cudaStream_t st)
 {
-    const int n = p.n_sp_cls[LA * 3 + LB];
+    const int c = LA * 3 + LB, n = p.n_sp_cls[c];
     if (n <= 0) return;
-    dim3 grid(n, (S / 2 + 63) / 64);
-    agen_kernel<LA, LB><<<grid, 64, 0, st>>>(p, p.sp_cls[LA * 3 + LB], g0, nb, S, w0, Astack, ld);
+    int goff = 0;
+    for (int k = 0; k < c; ++k) goff += agen_groups(p, k);
+    dim3 grid(agen_groups(p, c), (S / 2 + 63) / 64);
+    agen_kernel<LA, LB><<<grid, 64, 0, st>>>(p, p.sp_cls[c], n, g0, nb, S, w0, Astack, ld, Pp,
+                                              rho_part ? rho_part + (size_t)goff * S : nullptr);
 }
 int agen_launches(const LRParams &p)
 {
@@ -327,70 +354,47 @@ int agen_launches(const LRParams &p)
     for (int c = 0; c < 9; ++c) n += p.n_sp_cls[c] > 0;
     return n;
 }
-void launch_agen(const LRParams &p, int g0, int nb, int S, double w0, double *Astack, cudaStream_t st)
+static double *rho_partials(double *rho, int S);
+// rho (optional): rho_scratch_doubles(S, groups) doubles -- S results (filled by launch_rho_final) then the per-CTA partials
+void launch_agen(const LRParams &p, int g0, int nb, int S, double w0, double *Astack, const double *Pp, double *rho, cudaStream_t st)
 {
     if (p.U.nsp <= 0 || nb <= 0) return;
     const size_t ld = (size_t)p.Np * S;
-    launch_agen_class<0, 0>(p, g0, nb, S, w0, Astack, ld, st); launch_agen_class<0, 1>(p, g0, nb, S, w0, Astack, ld, st);
-    launch_agen_class<0, 2>(p, g0, nb, S, w0, Astack, ld, st); launch_agen_class<1, 0>(p, g0, nb, S, w0, Astack, ld, st);
-    launch_agen_class<1, 1>(p, g0, nb, S, w0, Astack, ld, st); launch_agen_class<1, 2>(p, g0, nb, S, w0, Astack, ld, st);
-    launch_agen_class<2, 0>(p, g0, nb, S, w0, Astack, ld, st); launch_agen_class<2, 1>(p, g0, nb, S, w0, Astack, ld, st);
-    launch_agen_class<2, 2>(p, g0, nb, S, w0, Astack, ld, st);
+    double *part = rho ? rho_partials(rho, S) : nullptr;
+#define AG(LA, LB) launch_agen_class<LA, LB>(p, g0, nb, S, w0, Astack, ld, Pp, part, st);
+    AG(0, 0) AG(0, 1) AG(0, 2) AG(1, 0) AG(1, 1) AG(1, 2) AG(2, 0) AG(2, 1) AG(2, 2)
+#undef AG
 }
 
-// rho'[slot] = sum_{mn} P'_mn A'_mn[slot]: one block per row m, threads over the (contiguous) slots and groups of
-// columns, then a fixed-order sum of the row partials (deterministic).  HBM-bound: streams the stored batch once.
-__global__ void __launch_bounds__(256) rho_reduce_kernel(const double *__restrict__ Pp, const double *__restrict__ Astack,
-                                                         size_t ld, int Np, int N, int S, double *__restrict__ part)
+// rho'[slot] = sum over the agen CTAs' partials part[g][slot], in two fixed-order stages (deterministic): RHO_NB blocks each
+// sum the partials g = b, b + RHO_NB, ... into part2[b][slot]; one block sums the RHO_NB rows.
+constexpr int RHO_NB = 148;
+__global__ void __launch_bounds__(128) rho_stage1_kernel(const double *__restrict__ part, int ngrp, int S, double *__restrict__ part2)
 {
-    __shared__ double sh[256];
-    const int m = blockIdx.x;
-    const int ngrp = 256 / S, grp = threadIdx.x / S, slot = threadIdx.x % S;      // S <= 128
-    double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
-    if (grp < ngrp) {
-        const double *a = Astack + (size_t)m * ld + slot;
-        const double *pr = Pp + (size_t)m * Np;
-        int n = grp;
-        for (; n + 3 * ngrp < N; n += 4 * ngrp) {
-            a0 = fma(pr[n], a[(size_t)n * S], a0);
-            a1 = fma(pr[n + ngrp], a[(size_t)(n + ngrp) * S], a1);
-            a2 = fma(pr[n + 2 * ngrp], a[(size_t)(n + 2 * ngrp) * S], a2);
-            a3 = fma(pr[n + 3 * ngrp], a[(size_t)(n + 3 * ngrp) * S], a3);
-        }
-        for (; n < N; n += ngrp) a0 = fma(pr[n], a[(size_t)n * S], a0);
-    }
-    sh[threadIdx.x] = (a0 + a1) + (a2 + a3);
-    __syncthreads();
-    if (threadIdx.x < S) {
-        double t = 0.0;
-        for (int g = 0; g < ngrp; ++g) t += sh[g * S + threadIdx.x];
-        part[(size_t)m * S + threadIdx.x] = t;
-    }
+    const int slot = threadIdx.x;
+    if (slot >= S) return;
+    double t0 = 0.0, t1 = 0.0;
+    int m = blockIdx.x;
+    for (; m + RHO_NB < ngrp; m += 2 * RHO_NB) { t0 += part[(size_t)m * S + slot]; t1 += part[(size_t)(m + RHO_NB) * S + slot]; }
+    if (m < ngrp) t0 += part[(size_t)m * S + slot];
+    part2[(size_t)blockIdx.x * S + slot] = t0 + t1;
 }
-// rho[slot] = sum_m part[m][slot]: 8 row groups per slot, summed in a fixed order
-__global__ void __launch_bounds__(1024) rho_final_kernel(const double *__restrict__ part, int N, int S, double *__restrict__ rho)
+__global__ void __launch_bounds__(128) rho_stage2_kernel(const double *__restrict__ part2, int S, double *__restrict__ rho)
 {
-    __shared__ double sh[1024];
-    const int slot = threadIdx.x % 128, grp = threadIdx.x / 128;
-    double t = 0.0;
-    if (slot < S)
-        for (int m = grp; m < N; m += 8) t += part[(size_t)m * S + slot];
-    sh[threadIdx.x] = t;
-    __syncthreads();
-    if (threadIdx.x < S) {
-        double r = 0.0;
-        for (int g = 0; g < 8; ++g) r += sh[g * 128 + threadIdx.x];
-        rho[threadIdx.x] = r;
-    }
+    const int slot = threadIdx.x;
+    if (slot >= S) return;
+    double r = 0.0;
+    for (int b = 0; b < RHO_NB; ++b) r += part2[(size_t)b * S + slot];
+    rho[slot] = r;
 }
-int rho_scratch_doubles(int S, int N) { return S * (N + 1); }
-// rho: S results followed by S*N row partials (rho_scratch_doubles)
-void launch_rho_reduce(const double *Pp, const double *Astack, int Np, int N, int S, double *rho, cudaStream_t st)
+// layout of the scratch: S results | RHO_NB * S stage-1 sums | ngroups * S partials of the agen CTAs
+int rho_scratch_doubles(int S, int ngroups) { return S * (1 + RHO_NB + ngroups); }
+static double *rho_partials(double *rho, int S) { return rho + (size_t)S * (1 + RHO_NB); }
+void launch_rho_final(const LRParams &p, int S, double *rho, cudaStream_t st)
 {
     if (S <= 0) return;
-    double *part = rho + S;
-    rho_reduce_kernel<<<N, 256, 0, st>>>(Pp, Astack, (size_t)Np * S, Np, N, S, part);
-    rho_final_kernel<<<1, 1024, 0, st>>>(part, N, S, rho);
+    rho_stage1_kernel<<<RHO_NB, 128, 0, st>>>(rho_partials(rho, S), agen_groups_total(p), S, rho + S);
+    rho_stage2_kernel<<<1, 128, 0, st>>>(rho + S, S, rho);
 }
 
 // Jacc[m][n] += sign * sum_slot A'[m][n][slot] rho'[slot]: one warp per matrix element, lanes over the slots
@@ -423,6 +427,8 @@ void launch_jlr_accum(const double *Astack, int Np, int N, int S, const double *
 // ---------------------------------------------------------------- FP64 tensor-core GEMM (A8, A9)
 namespace {
 constexpr int BM = 128, BN = 128, BK = 16;
+constexpr int NSTAGE = 4;     // cp.async ring: tiles t+1 .. t+3 are in flight while tile t is multiplied, one barrier per tile
+                              // (the kernel holds 166 registers x 256 threads: one CTA per SM, so nothing else hides the waits)
 constexpr int SA = BK + 4;    // row stride of the A tile [m][k]: (lane/4)*20 + lane%4 hits every bank pair twice
 constexpr int SB = BN + 8;    // row stride of the B tile [k][n]: (lane%4)*136 + lane/4 likewise
 
@@ -457,8 +463,8 @@ __global__ void __launch_bounds__(256) dgemm_kernel(int Kb, int nbatch, double a
     extern __shared__ __align__(16) double smem[];
     constexpr int A_TILE = TA ? BK * SB : BM * SA;
     constexpr int B_TILE = TB ? BN * SA : BK * SB;
-    double *As = smem;                       // [2][A_TILE]
-    double *Bs = smem + 2 * A_TILE;          // [2][B_TILE]
+    double *As = smem;                       // [NSTAGE][A_TILE]
+    double *Bs = smem + NSTAGE * A_TILE;     // [NSTAGE][B_TILE]
     const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
     const int wm = w >> 2, wn = w & 3;
     const int bm = blockIdx.y, bn = blockIdx.x, z = blockIdx.z;
@@ -517,16 +523,18 @@ __global__ void __launch_bounds__(256) dgemm_kernel(int Kb, int nbatch, double a
         asm volatile("cp.async.commit_group;\n" ::);
     };
 
-    if (ntile > 0) load_tile(0, 0);
+    // prologue: NSTAGE - 1 tiles in flight (empty commit groups keep the group count uniform)
+#pragma unroll
+    for (int t = 0; t < NSTAGE - 1; ++t) {
+        if (t < ntile) load_tile(t, t);
+        else asm volatile("cp.async.commit_group;\n" ::);
+    }
     for (int t = 0; t < ntile; ++t) {
-        const int buf = t & 1;
-        if (t + 1 < ntile) {
-            load_tile(t + 1, buf ^ 1);
-            asm volatile("cp.async.wait_group 1;\n" ::);
-        } else {
-            asm volatile("cp.async.wait_group 0;\n" ::);
-        }
-        __syncthreads();
+        const int buf = t % NSTAGE;
+        asm volatile("cp.async.wait_group %0;\n" ::"n"(NSTAGE - 2));       // tile t has landed (for this thread)
+        __syncthreads();                                                    // ... for all; and everyone is done with tile t-1
+        if (t + NSTAGE - 1 < ntile) load_tile(t + NSTAGE - 1, (t + NSTAGE - 1) % NSTAGE);   // into the buffer of tile t-1
+        else asm volatile("cp.async.commit_group;\n" ::);
         const double *as = TA ? As + buf * A_TILE + (lane & 3) * SB + wm * 64 + (lane >> 2)
                               : As + buf * A_TILE + (wm * 64 + (lane >> 2)) * SA + (lane & 3);
         const double *bs = TB ? Bs + buf * B_TILE + (wn * 32 + (lane >> 2)) * SA + (lane & 3)
@@ -543,7 +551,6 @@ __global__ void __launch_bounds__(256) dgemm_kernel(int Kb, int nbatch, double a
 #pragma unroll
                 for (int j = 0; j < 4; ++j) dmma(acc[i][j][0], acc[i][j][1], a[i], b[j]);
         }
-        __syncthreads();
     }
 #pragma unroll
     for (int i = 0; i < 8; ++i)
@@ -563,8 +570,8 @@ __global__ void __launch_bounds__(256) dgemm_kernel(int Kb, int nbatch, double a
 }
 
 namespace {
-constexpr int smemN = 2 * (BM * SA + BK * SB) * (int)sizeof(double), smemT = 2 * (2 * BK * SB) * (int)sizeof(double);
-constexpr int smemNT = 2 * (BM * SA + BN * SA) * (int)sizeof(double);
+constexpr int smemN = NSTAGE * (BM * SA + BK * SB) * (int)sizeof(double), smemT = NSTAGE * (2 * BK * SB) * (int)sizeof(double);
+constexpr int smemNT = NSTAGE * (BM * SA + BN * SA) * (int)sizeof(double);
 }  // namespace
 // the opt-in is per device: pbc_jk_create calls this for the handle's device
 void dgemm_set_attributes()
@@ -619,55 +626,80 @@ __global__ void chol_init_kernel(const double *__restrict__ Pp, int N, int Np, d
     }
 }
 
-// step k: every block finds the pivot (largest residual diagonal, lowest index on ties) on its own, then forms its
-// rows of column k.  d_in / d_out alternate between steps so no block reads what another writes.
-__global__ void __launch_bounds__(128) chol_step_kernel(int k, const double *__restrict__ Pp, int N, int Np,
-                                                        double *__restrict__ LT, const double *__restrict__ d_in,
-                                                        double *__restrict__ d_out, int *dyn, const double *__restrict__ dscal)
+// All steps in ONE cooperative launch (the blocks are co-resident, so they may wait on one another): at step k every
+// block finds the pivot (largest residual diagonal, lowest index on ties) on its own from the same d array, forms its
+// rows of column k, and the grid meets at a barrier.  d_a / d_b alternate between steps so no block reads what another
+// writes within a step; the stop decision is taken from data every block sees identically (no flag written and read
+// in the same step).  bar: two ints (arrival count, generation), zeroed before the launch.
+__device__ __forceinline__ void chol_grid_barrier(unsigned *bar, unsigned nblocks)
 {
-    if (dyn[2]) return;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        volatile unsigned *gen = bar + 1;
+        const unsigned g = *gen;
+        __threadfence();
+        if (atomicAdd(bar, 1u) == nblocks - 1) {
+            *bar = 0;
+            __threadfence();
+            atomicAdd((unsigned *)bar + 1, 1u);
+        } else {
+            while (*gen == g) { }
+        }
+        __threadfence();
+    }
+    __syncthreads();
+}
+
+__global__ void __launch_bounds__(128) chol_all_kernel(const double *__restrict__ Pp, int N, int Np, double *__restrict__ LT,
+                                                       double *__restrict__ dbuf, int *dyn, const double *__restrict__ dscal,
+                                                       unsigned *bar)
+{
     __shared__ double sv[4];
     __shared__ int si[4];
-    double best = -1.0;
-    int bi = 0x7fffffff;
-    for (int i = threadIdx.x; i < N; i += 128) {
-        const double v = d_in[i];
-        if (v > best) { best = v; bi = i; }
-    }
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) {
-        const double ov = __shfl_xor_sync(0xffffffffu, best, o);
-        const int oi = __shfl_xor_sync(0xffffffffu, bi, o);
-        if (ov > best || (ov == best && oi < bi)) { best = ov; bi = oi; }
-    }
-    if ((threadIdx.x & 31) == 0) { sv[threadIdx.x >> 5] = best; si[threadIdx.x >> 5] = bi; }
-    __syncthreads();
-    best = sv[0]; bi = si[0];
-#pragma unroll
-    for (int w = 1; w < 4; ++w)
-        if (sv[w] > best || (sv[w] == best && si[w] < bi)) { best = sv[w]; bi = si[w]; }
-    if (!(best > 1e-13 * dscal[0]) || !(best > 0.0)) {
-        if (blockIdx.x == 0 && threadIdx.x == 0) dyn[2] = 1;
-        return;
-    }
-    const int i = blockIdx.x * 128 + threadIdx.x;
-    if (i < N) {
-        double s0 = Pp[(size_t)bi * Np + i], s1 = 0.0, s2 = 0.0, s3 = 0.0;
-        int j = 0;
-        for (; j + 4 <= k; j += 4) {
-            s0 = fma(-LT[(size_t)j * Np + i], LT[(size_t)j * Np + bi], s0);
-            s1 = fma(-LT[(size_t)(j + 1) * Np + i], LT[(size_t)(j + 1) * Np + bi], s1);
-            s2 = fma(-LT[(size_t)(j + 2) * Np + i], LT[(size_t)(j + 2) * Np + bi], s2);
-            s3 = fma(-LT[(size_t)(j + 3) * Np + i], LT[(size_t)(j + 3) * Np + bi], s3);
+    const double dmax = dscal[0];
+    int k = 0;
+    for (; k < N; ++k) {
+        const double *d_in = dbuf + (size_t)(k & 1) * Np;
+        double *d_out = dbuf + (size_t)((k + 1) & 1) * Np;
+        double best = -1.0;
+        int bi = 0x7fffffff;
+        for (int i = threadIdx.x; i < N; i += 128) {
+            const double v = __ldcg(d_in + i);               // written by other blocks in the previous step: read through L2
+            if (v > best) { best = v; bi = i; }
         }
-        for (; j < k; ++j) s0 = fma(-LT[(size_t)j * Np + i], LT[(size_t)j * Np + bi], s0);
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            const double ov = __shfl_xor_sync(0xffffffffu, best, o);
+            const int oi = __shfl_xor_sync(0xffffffffu, bi, o);
+            if (ov > best || (ov == best && oi < bi)) { best = ov; bi = oi; }
+        }
+        if ((threadIdx.x & 31) == 0) { sv[threadIdx.x >> 5] = best; si[threadIdx.x >> 5] = bi; }
+        __syncthreads();
+        best = sv[0]; bi = si[0];
+#pragma unroll
+        for (int w = 1; w < 4; ++w)
+            if (sv[w] > best || (sv[w] == best && si[w] < bi)) { best = sv[w]; bi = si[w]; }
+        __syncthreads();
+        if (!(best > 1e-13 * dmax) || !(best > 0.0)) break;  // same decision in every block
         const double root = sqrt(best);
-        double v = ((s0 + s1) + (s2 + s3)) / root;
-        if (i == bi) v = root;
-        LT[(size_t)k * Np + i] = v;
-        d_out[i] = (i == bi) ? 0.0 : d_in[i] - v * v;
+        for (int i = blockIdx.x * 128 + threadIdx.x; i < N; i += gridDim.x * 128) {
+            double s0 = Pp[(size_t)bi * Np + i], s1 = 0.0, s2 = 0.0, s3 = 0.0;
+            int j = 0;
+            for (; j + 4 <= k; j += 4) {
+                s0 = fma(-LT[(size_t)j * Np + i], __ldcg(LT + (size_t)j * Np + bi), s0);
+                s1 = fma(-LT[(size_t)(j + 1) * Np + i], __ldcg(LT + (size_t)(j + 1) * Np + bi), s1);
+                s2 = fma(-LT[(size_t)(j + 2) * Np + i], __ldcg(LT + (size_t)(j + 2) * Np + bi), s2);
+                s3 = fma(-LT[(size_t)(j + 3) * Np + i], __ldcg(LT + (size_t)(j + 3) * Np + bi), s3);
+            }
+            for (; j < k; ++j) s0 = fma(-LT[(size_t)j * Np + i], __ldcg(LT + (size_t)j * Np + bi), s0);
+            double v = ((s0 + s1) + (s2 + s3)) / root;
+            if (i == bi) v = root;
+            LT[(size_t)k * Np + i] = v;                      // row k, element i: only this thread ever writes or reads (own i)
+            d_out[i] = (i == bi) ? 0.0 : __ldcg(d_in + i) - v * v;
+        }
+        chol_grid_barrier(bar, gridDim.x);
     }
-    if (blockIdx.x == 0 && threadIdx.x == 0) dyn[0] = k + 1;
+    if (blockIdx.x == 0 && threadIdx.x == 0) { dyn[0] = k; dyn[2] = 1; }
 }
 
 // max |P' - L L^T| over the lower-triangular tiles (R holds L L^T there)
@@ -731,10 +763,18 @@ void launch_factor_density(const double *Pp, int N, int Np, double *LT, double *
 {
     cudaMemsetAsync(LT, 0, (size_t)Np * Np * sizeof(double), st);
     chol_init_kernel<<<1, 1024, 0, st>>>(Pp, N, Np, dbuf, dyn, dscal);
-    const int nblk = (N + 127) / 128;
-    for (int k = 0; k < N; ++k)
-        chol_step_kernel<<<nblk, 128, 0, st>>>(k, Pp, N, Np, LT, dbuf + (size_t)(k & 1) * Np, dbuf + (size_t)((k + 1) & 1) * Np, dyn,
-                                               dscal);
+    // one cooperative launch for all steps (at most one block per 128 rows, capped by what is co-resident)
+    {
+        int dev = 0, nsm = 1, per_sm = 1;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, chol_all_kernel, 128, 0);
+        int nblk = std::min((N + 127) / 128, nsm * std::max(per_sm, 1));
+        unsigned *bar = reinterpret_cast<unsigned *>(dyn + 4);
+        cudaMemsetAsync(bar, 0, 2 * sizeof(unsigned), st);
+        void *args[] = {(void *)&Pp, (void *)&N, (void *)&Np, (void *)&LT, (void *)&dbuf, (void *)&dyn, (void *)&dscal, (void *)&bar};
+        cudaLaunchCooperativeKernel((const void *)chol_all_kernel, dim3(nblk), dim3(128), args, 0, st);
+    }
     // residual: scratch = L L^T on the lower-triangular tiles
     GemmArgs g;
     g.M = Np; g.Nc = Np; g.Kb = Np; g.nbatch = 1; g.alpha = 1.0; g.A = LT; g.lda = Np; g.strideA = 0; g.B = LT; g.ldb = Np;
@@ -746,7 +786,7 @@ void launch_factor_density(const double *Pp, int N, int Np, double *LT, double *
     const size_t tot = (size_t)Np * Np;
     chol_fallback_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, st>>>(Pp, N, Np, LT, dyn, dscal);
 }
-int factor_density_launches(int N) { return 1 + N + 3; }
+int factor_density_launches(int) { return 1 + 1 + 3; }
 
 // ---------------------------------------------------------------- finalise (A10)
 __global__ void finalize_j_kernel(const double *__restrict__ Jsr, const double *__restrict__ Jlr, int N,

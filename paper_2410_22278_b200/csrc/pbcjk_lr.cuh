@@ -36,11 +36,13 @@ void launch_j_backtransform(const PairListU &U, const ShellInfo &sh, const doubl
 // A'(G) = sqrt(w) rho_mn(G) for G in [g0, g0+nb): real and imaginary parts as slots 2g, 2g+1 of the stack
 //   A'[row*ld + col*S + slot], ld = Np*S, S >= 2*nb a multiple of 16 (slots past 2*nb are written as 0).
 // g0 < 0: the single G = 0 slot with weight `w0` (overlap S, eq 21) in slot 0.
-void launch_agen(const LRParams &p, int g0, int nb, int S, double w0, double *Astack, cudaStream_t st);
+// With `rho` (rho_scratch_doubles(S, agen_groups_total) doubles) and the density Pp the kernels also leave the partial sums
+// of rho'[slot] = sum P' o A'[slot] there; launch_rho_final reduces them into rho[0..S).
+void launch_agen(const LRParams &p, int g0, int nb, int S, double w0, double *Astack, const double *Pp, double *rho, cudaStream_t st);
 int agen_launches(const LRParams &p);
-// rho'[slot] = sum P' o A'[slot]; rho must hold rho_scratch_doubles(S, N) doubles (results, then row partials)
-int rho_scratch_doubles(int S, int N);
-void launch_rho_reduce(const double *Pp, const double *Astack, int Np, int N, int S, double *rho, cudaStream_t st);
+int agen_groups_total(const LRParams &p);
+int rho_scratch_doubles(int S, int ngroups);
+void launch_rho_final(const LRParams &p, int S, double *rho, cudaStream_t st);
 // Jacc[m][n] += sign * sum_slot A'[m][n][slot] rho'[slot]
 void launch_jlr_accum(const double *Astack, int Np, int N, int S, const double *rho, double sign, double *Jacc, cudaStream_t st);
 // C[z][M x Nc] (ldc) = beta*C + alpha * sum_b op(A_b)[M x Kb] B_b[Kb x Nc](ldb) over the batches of split z;
@@ -61,10 +63,11 @@ struct GemmArgs {
 };
 void launch_dgemm(const GemmArgs &g, cudaStream_t st);
 // P' = L L^T (pivoted Cholesky, device-side rank in dyn[0]) with the dense fallback L = P' (dyn[1] = 1);
-// LT: Np x Np (row k = column k of L), dbuf: 2*Np, dyn: 4 ints, dscal: 2 doubles, scratch: Np x Np
+// LT: Np x Np (row k = column k of L), dbuf: 2*Np, dyn: 8 ints (4 + the grid barrier of the one-launch factorisation),
+// dscal: 2 doubles, scratch: Np x Np
 void launch_factor_density(const double *Pp, int N, int Np, double *LT, double *dbuf, int *dyn, double *dscal, double *scratch,
                            cudaStream_t st);
-int factor_density_launches(int N);
+int factor_density_launches(int N);     // kernels launch_factor_density enqueues
 // occupied-orbital entry point: P = C C^T (N x N, unscaled) and the factor LT = (f C)^T with rank nocc (dyn as above)
 void launch_density_from_orbitals(const double *C, int N, int nocc, double *P, cudaStream_t st);
 void launch_factor_from_orbitals(const double *C, int N, int nocc, int Np, const double *fcomp, double *LT, int *dyn, cudaStream_t st);
