@@ -157,7 +157,7 @@ def _ncu_traffic(kernel):
 
 def h_nb(st, n):
     """G vectors per reciprocal-space batch as pbc_jk_create sizes them (stacks <= 12 GB, at most 64)"""
-    np_ = ((n + 127) // 128) * 128
+    np_ = ((n + 63) // 64) * 64
     return max(1, min(64, int(12.0e9 // (np_ * np_ * 16)), max(st["n_g"], 1)))
 
 

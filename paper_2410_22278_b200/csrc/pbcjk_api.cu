@@ -60,7 +60,7 @@ struct HostPair {
 struct pbc_jk {
     std::string err;
     DevPool pool;
-    int N = 0, Np = 0, nshell = 0, natom = 0, nG = 0;
+    int N = 0, Np = 0, Npt = 0, nshell = 0, natom = 0, nG = 0;   // Np: N padded to 64 (strides, GEMM k and n); Npt: to the 128-row GEMM tiles
     int device = 0, nsm = 148;           // the CUDA device the handle lives on (current device at create)
     int parts = 7;
     pbc_cutoffs cut{};
@@ -262,7 +262,8 @@ int setup(pbc_jk *h, const pbc_cell *cell, const pbc_atoms *atoms, const pbc_she
         nprim_tot = std::max(nprim_tot, shells->prim_off[s] + shells->nprim[s]);
     }
     h->N = nbf;
-    h->Np = ((nbf + 127) / 128) * 128;
+    h->Np = ((nbf + 63) / 64) * 64;
+    h->Npt = ((nbf + 127) / 128) * 128;
     std::vector<double> cn(nprim_tot, 0.0);
     for (int s = 0; s < ns; ++s)
         for (int k = 0; k < shells->nprim[s]; ++k) {
@@ -706,7 +707,7 @@ int setup(pbc_jk *h, const pbc_cell *cell, const pbc_atoms *atoms, const pbc_she
     }
     // ---- workspaces ----
     {
-        const size_t Np = h->Np, N = nbf;
+        const size_t Np = h->Np, Npt = h->Npt, N = nbf;
         // G batch: A' and Y stacks of Np x 2nb x Np doubles each, at most 12 GB per stack (180 GB HBM3e per GPU)
         int nb = cut.lr_g_batch > 0 ? cut.lr_g_batch : (int)std::min<double>(64.0, std::floor(12.0e9 / (double)(Np * Np * 16)));
         nb = std::max(1, std::min(std::min(nb, 64), std::max(h->nG, 1)));      // the slot kernels hold at most 128 slots
@@ -717,7 +718,7 @@ int setup(pbc_jk *h, const pbc_cell *cell, const pbc_atoms *atoms, const pbc_she
         // fill whole waves of one CTA per SM
         {
             const int nsm = h->nsm;
-            const long tiles = (long)(Np / 128) * (Np / 128 + 1) / 2;
+            const long tiles = (long)(Npt / 128) * (Npt / 128 + 1) / 2;
             double best = 0.0;
             h->nsplit = 1;
             for (int ns = 1; ns <= 8; ++ns) {
@@ -735,11 +736,13 @@ int setup(pbc_jk *h, const pbc_cell *cell, const pbc_atoms *atoms, const pbc_she
         CK(pool.alloc(&h->Dt, (size_t)nherm(4) * h->KJ.dstride));
         CK(pool.alloc(&h->Jt, (size_t)nherm(4) * std::max(h->U.n, 1)));
         CK(pool.alloc(&h->Jsr, N * N)); CK(pool.alloc(&h->Jlr, N * N)); CK(pool.alloc(&h->Ksr, N * N));
-        CK(pool.alloc(&h->Klr, (size_t)h->nsplit * Np * Np));
-        CK(pool.alloc(&h->Astack, Np * h->ld)); CK(cudaMemset(h->Astack, 0, Np * h->ld * 8));
-        CK(pool.alloc(&h->Zstack, Np * h->ld));
+        CK(pool.alloc(&h->Klr, (size_t)h->nsplit * Npt * Npt));
+        // the GEMM row tiles are 128 high: the last one may reach up to 64 rows past Np (rows that are read or written but never
+        // used), hence Npt rows
+        CK(pool.alloc(&h->Astack, Npt * h->ld)); CK(cudaMemset(h->Astack, 0, Npt * h->ld * 8));
+        CK(pool.alloc(&h->Zstack, Npt * h->ld)); CK(cudaMemset(h->Zstack, 0, Npt * h->ld * 8));
         CK(pool.alloc(&h->rho, (size_t)rho_scratch_doubles(h->Smax, agen_groups_total(h->lr))));
-        CK(pool.alloc(&h->LT, Np * Np)); CK(pool.alloc(&h->chol_d, 2 * Np)); CK(pool.alloc(&h->chol_s, 2));
+        CK(pool.alloc(&h->LT, Npt * Np)); CK(pool.alloc(&h->chol_d, 2 * Np)); CK(pool.alloc(&h->chol_s, 2));
         CK(pool.alloc(&h->chol_dyn, 8));      // rank, fallback flag, done, -, grid barrier (2)
         CK(pool.alloc(&h->hostP, N * N)); CK(pool.alloc(&h->hostJ, N * N)); CK(pool.alloc(&h->hostK, N * N));
         for (auto &e : h->ev) CK(cudaEventCreate(&e));
@@ -870,7 +873,7 @@ static int build_impl(pbc_jk *h, const double *P, const double *Corb, int nocc, 
         if (dev != h->device) return fail(h, PBC_JK_ERR_INVALID_ARG, "the handle was created on another CUDA device than the current one");
     }
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    const int N = h->N, Np = h->Np;
+    const int N = h->N, Np = h->Np, Npt = h->Npt;
     const size_t NN = (size_t)N * N;
     const bool doSR = h->parts & 1, doLR = h->parts & 2, doSELF = (h->parts & 4) && h->shard_rank == 0;
     const bool prof = h->profile;
@@ -962,15 +965,15 @@ static int build_impl(pbc_jk *h, const double *P, const double *Corb, int nocc, 
     // ---- A7/A8: reciprocal space, batches of G (on the caller's stream) ----
     const bool needJlr = J && (doLR || doSELF), needKlr = K && (doLR || doSELF);
     if (J) CK(cudaMemsetAsync(h->Jlr, 0, NN * 8, st));
-    if (K) CK(cudaMemsetAsync(h->Klr, 0, (size_t)h->nsplit * Np * Np * 8, st));
-    const size_t strideK = (size_t)Np * Np;
+    if (K) CK(cudaMemsetAsync(h->Klr, 0, (size_t)h->nsplit * Npt * Npt * 8, st));
+    const size_t strideK = (size_t)Npt * Npt;
     // K^LR = sum_slots Y^T Y with Y = L^T A', P' = L L^T (device-side rank; dense fallback inside the same kernels)
     if (needKlr) {
         if (Corb) {                      // the orbitals are the factor: no decomposition
-            launch_factor_from_orbitals(Corb, N, nocc, Np, h->fcomp, h->LT, h->chol_dyn, st);
+            launch_factor_from_orbitals(Corb, N, nocc, Np, Npt, h->fcomp, h->LT, h->chol_dyn, st);
             nl += 1;
         } else {
-            launch_factor_density(h->Pp, N, Np, h->LT, h->chol_d, h->chol_dyn, h->chol_s, h->Zstack, st);
+            launch_factor_density(h->Pp, N, Np, Npt, h->LT, h->chol_d, h->chol_dyn, h->chol_s, h->Zstack, st);
             nl += factor_density_launches(N);
         }
     }
@@ -982,13 +985,13 @@ static int build_impl(pbc_jk *h, const double *P, const double *Corb, int nocc, 
         const bool tg = prof && 2 * (size_t)h->n_evG + 1 < h->evG.size();
         if (tg) cudaEventRecord(h->evG[2 * h->n_evG], st);
         GemmArgs g1;
-        g1.M = Np; g1.Nc = Np * S; g1.Kb = Np; g1.nbatch = 1; g1.A = h->LT; g1.lda = Np; g1.B = h->Astack; g1.ldb = ldS;
+        g1.M = Npt; g1.Nc = Np * S; g1.Kb = Np; g1.nbatch = 1; g1.A = h->LT; g1.lda = Np; g1.B = h->Astack; g1.ldb = ldS;
         g1.C = h->Zstack; g1.ldc = ldS; g1.dyn = h->chol_dyn; g1.use_dyn = 1;
         launch_dgemm(g1, st);
         GemmArgs g2;
-        g2.M = Np; g2.Nc = Np; g2.Kb = S; g2.nbatch = Np; g2.alpha = alpha; g2.transB = true;
+        g2.M = Npt; g2.Nc = Npt; g2.Kb = S; g2.nbatch = Np; g2.alpha = alpha; g2.transB = true;
         g2.A = h->Zstack; g2.lda = S; g2.strideA = ldS; g2.B = h->Zstack; g2.ldb = S; g2.strideB = ldS;
-        g2.B_alt = h->Astack; g2.beta = 1.0; g2.C = h->Klr; g2.ldc = Np; g2.strideC = strideK; g2.nsplit = nsplit;
+        g2.B_alt = h->Astack; g2.beta = 1.0; g2.C = h->Klr; g2.ldc = Npt; g2.strideC = strideK; g2.nsplit = nsplit;
         g2.dyn = h->chol_dyn; g2.use_dyn = 4 | 8; g2.lower_only = 1;
         launch_dgemm(g2, st);
         if (tg) { cudaEventRecord(h->evG[2 * h->n_evG + 1], st); ++h->n_evG; }
@@ -1035,7 +1038,7 @@ static int build_impl(pbc_jk *h, const double *P, const double *Corb, int nocc, 
     // ---- A10 ----
     if (J) launch_finalize_j(doSR ? h->Jsr : nullptr, h->Jlr, N, h->fcomp, J, st);
     if (K)
-        launch_finalize_k(doSR ? h->Ksr : nullptr, h->sh, h->Klr, h->nsplit, strideK, Np, N, h->fcomp,
+        launch_finalize_k(doSR ? h->Ksr : nullptr, h->sh, h->Klr, h->nsplit, strideK, Npt, N, h->fcomp,
                           h->shell_of_ao, K, st);
     nl += (J ? 1 : 0) + (K ? 1 : 0);
     CK(cudaEventRecord(h->ev[5], st));

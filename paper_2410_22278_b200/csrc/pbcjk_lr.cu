@@ -703,12 +703,12 @@ __global__ void __launch_bounds__(128) chol_all_kernel(const double *__restrict_
 }
 
 // max |P' - L L^T| over the lower-triangular tiles (R holds L L^T there)
-__global__ void chol_residual_kernel(const double *__restrict__ Pp, const double *__restrict__ R, int N, int Np,
+__global__ void chol_residual_kernel(const double *__restrict__ Pp, const double *__restrict__ R, int N, int Np, int ldR,
                                      unsigned long long *resbits)
 {
     const int n = blockIdx.x * blockDim.x + threadIdx.x, m = blockIdx.y;
     double v = 0.0;
-    if (n < N && (n / BN) <= (m / BM)) v = fabs(Pp[(size_t)m * Np + n] - R[(size_t)m * Np + n]);
+    if (n < N && (n / BN) <= (m / BM)) v = fabs(Pp[(size_t)m * Np + n] - R[(size_t)m * ldR + n]);
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, o));
     if ((threadIdx.x & 31) == 0 && v > 0.0) atomicMax(resbits, (unsigned long long)__double_as_longlong(v));
@@ -751,17 +751,18 @@ void launch_density_from_orbitals(const double *C, int N, int nocc, double *P, c
     dim3 grid((N + 127) / 128, N);
     density_from_orbitals_kernel<<<grid, 128, 0, st>>>(C, N, nocc, P);
 }
-void launch_factor_from_orbitals(const double *C, int N, int nocc, int Np, const double *fcomp, double *LT, int *dyn, cudaStream_t st)
+void launch_factor_from_orbitals(const double *C, int N, int nocc, int Np, int Npt, const double *fcomp, double *LT, int *dyn,
+                                 cudaStream_t st)
 {
-    cudaMemsetAsync(LT, 0, (size_t)Np * Np * sizeof(double), st);
+    cudaMemsetAsync(LT, 0, (size_t)Npt * Np * sizeof(double), st);
     dim3 grid((N + 127) / 128, nocc);
     factor_from_orbitals_kernel<<<grid, 128, 0, st>>>(C, N, nocc, Np, fcomp, LT, dyn);
 }
 
-void launch_factor_density(const double *Pp, int N, int Np, double *LT, double *dbuf, int *dyn, double *dscal, double *scratch,
-                           cudaStream_t st)
+void launch_factor_density(const double *Pp, int N, int Np, int Npt, double *LT, double *dbuf, int *dyn, double *dscal,
+                           double *scratch, cudaStream_t st)
 {
-    cudaMemsetAsync(LT, 0, (size_t)Np * Np * sizeof(double), st);
+    cudaMemsetAsync(LT, 0, (size_t)Npt * Np * sizeof(double), st);
     chol_init_kernel<<<1, 1024, 0, st>>>(Pp, N, Np, dbuf, dyn, dscal);
     // one cooperative launch for all steps (at most one block per 128 rows, capped by what is co-resident)
     {
@@ -777,12 +778,14 @@ void launch_factor_density(const double *Pp, int N, int Np, double *LT, double *
     }
     // residual: scratch = L L^T on the lower-triangular tiles
     GemmArgs g;
-    g.M = Np; g.Nc = Np; g.Kb = Np; g.nbatch = 1; g.alpha = 1.0; g.A = LT; g.lda = Np; g.strideA = 0; g.B = LT; g.ldb = Np;
-    g.strideB = 0; g.beta = 0.0; g.C = scratch; g.ldc = Np; g.strideC = 0; g.nsplit = 1; g.transA = true; g.dyn = dyn;
+    // (128 x 128 tiles over Npt; the part of a tile past Np multiplies whatever follows in LT into rows / columns of the
+    //  scratch that nothing reads)
+    g.M = Npt; g.Nc = Npt; g.Kb = Np; g.nbatch = 1; g.alpha = 1.0; g.A = LT; g.lda = Np; g.strideA = 0; g.B = LT; g.ldb = Np;
+    g.strideB = 0; g.beta = 0.0; g.C = scratch; g.ldc = Npt; g.strideC = 0; g.nsplit = 1; g.transA = true; g.dyn = dyn;
     g.use_dyn = 2; g.lower_only = 1;
     launch_dgemm(g, st);
     dim3 grid((N + 127) / 128, N);
-    chol_residual_kernel<<<grid, 128, 0, st>>>(Pp, scratch, N, Np, (unsigned long long *)(dscal + 1));
+    chol_residual_kernel<<<grid, 128, 0, st>>>(Pp, scratch, N, Np, Npt, (unsigned long long *)(dscal + 1));
     const size_t tot = (size_t)Np * Np;
     chol_fallback_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, st>>>(Pp, N, Np, LT, dyn, dscal);
 }

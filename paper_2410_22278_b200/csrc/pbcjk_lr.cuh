@@ -9,7 +9,7 @@ struct LRParams {
     PairListU U;
     ShellInfo sh;
     Lattice lat;
-    int N, Np;                 // basis size and its padded size (multiple of 128)
+    int N, Np;                 // basis size and its padded size (multiple of 64)
     const double *fcomp;       // [N] per-component factor (1 or sqrt 3)
     const double *Gx, *Gy, *Gz, *Gw;   // half-sphere G list, Gw = sqrt(2 * 4 pi/(Omega G^2) exp(-G^2/4w^2))
     const int *sp_cls[9];      // shell pairs of U by class (l_A*3 + l_B): one agen_kernel instantiation each
@@ -46,7 +46,8 @@ void launch_rho_final(const LRParams &p, int S, double *rho, cudaStream_t st);
 // Jacc[m][n] += sign * sum_slot A'[m][n][slot] rho'[slot]
 void launch_jlr_accum(const double *Astack, int Np, int N, int S, const double *rho, double sign, double *Jacc, cudaStream_t st);
 // C[z][M x Nc] (ldc) = beta*C + alpha * sum_b op(A_b)[M x Kb] B_b[Kb x Nc](ldb) over the batches of split z;
-// M, Nc multiples of 128, Kb of 16; grid.z = nsplit partial results C + z*strideC over disjoint batch ranges.
+// M, Nc multiples of 128, Kb of 16 (operand rows/columns past the logical size may alias the following memory: the
+// affected result rows/columns are never read); grid.z = nsplit partial results C + z*strideC over disjoint batch ranges.
 // See dgemm_kernel in pbcjk_lr.cu for transA / dyn / lower_only.
 struct GemmArgs {
     int M = 0, Nc = 0, Kb = 0, nbatch = 1;
@@ -65,12 +66,14 @@ void launch_dgemm(const GemmArgs &g, cudaStream_t st);
 // P' = L L^T (pivoted Cholesky, device-side rank in dyn[0]) with the dense fallback L = P' (dyn[1] = 1);
 // LT: Np x Np (row k = column k of L), dbuf: 2*Np, dyn: 8 ints (4 + the grid barrier of the one-launch factorisation),
 // dscal: 2 doubles, scratch: Np x Np
-void launch_factor_density(const double *Pp, int N, int Np, double *LT, double *dbuf, int *dyn, double *dscal, double *scratch,
-                           cudaStream_t st);
+// Npt = N padded to the 128-row GEMM tiles (LT holds Npt rows, the scratch Npt x Npt)
+void launch_factor_density(const double *Pp, int N, int Np, int Npt, double *LT, double *dbuf, int *dyn, double *dscal,
+                           double *scratch, cudaStream_t st);
 int factor_density_launches(int N);     // kernels launch_factor_density enqueues
 // occupied-orbital entry point: P = C C^T (N x N, unscaled) and the factor LT = (f C)^T with rank nocc (dyn as above)
 void launch_density_from_orbitals(const double *C, int N, int nocc, double *P, cudaStream_t st);
-void launch_factor_from_orbitals(const double *C, int N, int nocc, int Np, const double *fcomp, double *LT, int *dyn, cudaStream_t st);
+void launch_factor_from_orbitals(const double *C, int N, int nocc, int Np, int Npt, const double *fcomp, double *LT, int *dyn,
+                                 cudaStream_t st);
 // out = f f (sum of parts), symmetrised; see pbcjk_lr.cu
 void launch_finalize_j(const double *Jsr, const double *Jlr, int N, const double *fcomp, double *J, cudaStream_t st);
 void launch_finalize_k(const double *Ksr, const ShellInfo &sh, const double *Klr, int nsplit, size_t strideK, int Np,
