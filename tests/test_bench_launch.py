@@ -1,6 +1,6 @@
-"""The N > 1 launch path of bench.py on CPU (the path itself is "replicas only": there is no
-data-path collective to test).  Under torchrun with two processes the reference arm must run on rank 0 alone and
-print exactly one JSON line; the flop model of the roofline is checked against hand counts."""
+"""The N > 1 launch path of bench.py on CPU: under torchrun with two processes the reference arm must run on rank 0 alone
+and print exactly one JSON line (the all-reduce of the sharded build is covered by tests/test_shard_allreduce.py); the
+flop model of the roofline is checked against hand counts."""
 import json
 import os
 import subprocess

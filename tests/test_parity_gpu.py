@@ -335,3 +335,46 @@ def test_orbital_entry_point(torch_cuda, oracle_mod, name):
         assert h.stats()["rank_p"] == wl.n_occ
     assert np.abs(J.cpu().numpy() - ref["J"]).max() < TOL and np.abs(K.cpu().numpy() - ref["K"]).max() < TOL
     assert (J - J2).abs().max().item() < 1e-11 and (K - K2).abs().max().item() < 1e-11
+
+
+def test_entry_point_argument_errors(torch_cuda):
+    """The newer entry points refuse bad arguments with a status and a message, never a crash."""
+    from paper_2410_22278_b200 import workloads
+    from paper_2410_22278_b200.binding import PbcJK, PbcJKError, load
+    torch = torch_cuda
+    wl = workloads.get("tiny")
+    lib = load()
+    with PbcJK(wl) as h:
+        n = h.nbf
+        C = torch.zeros((n, 2), dtype=torch.float64, device="cuda")
+        J = torch.empty((n, n), dtype=torch.float64, device="cuda")
+        assert lib.pbc_jk_build_orbitals(h._h, None, 2, J.data_ptr(), None, None) == -1
+        assert lib.pbc_jk_build_orbitals(h._h, C.data_ptr(), 0, J.data_ptr(), None, None) == -1
+        assert lib.pbc_jk_build_orbitals(h._h, C.data_ptr(), n + 1, J.data_ptr(), None, None) == -1
+        assert b"nocc" in lib.pbc_jk_last_error(h._h)
+        assert lib.pbc_jk_one_electron(h._h, None, None, J.data_ptr(), None, None) == -1
+        assert lib.pbc_jk_set_shard(h._h, 2, 2) == -1 and lib.pbc_jk_set_shard(h._h, 0, 0) == -1
+        assert lib.pbc_jk_set_shard(h._h, 1, 2) == 0 and lib.pbc_jk_set_shard(h._h, 0, 1) == 0
+        with pytest.raises(ValueError):
+            h.build_orbitals(C.float(), J)
+        # a density outside the validated range of the packed lattice indices is reported, not silently mis-summed
+        P = torch.eye(n, dtype=torch.float64, device="cuda") * 1e7
+        h.build(P, J, None)
+        with pytest.raises(PbcJKError) as ei:
+            h.stats()
+        assert ei.value.code == -4
+
+
+def test_single_s_function_cell(torch_cuda, oracle_mod):
+    """Smallest possible input: one s primitive in a cube (every list has one entry, every class but (ss|ss) is empty)."""
+    from paper_2410_22278_b200 import workloads as W
+    wl = W.Workload(name="one", cell=np.eye(3) * 7.0, xyz=np.array([[0.3, 0.2, 0.1]]), sh_atom=np.zeros(1, np.int32),
+                    sh_l=np.zeros(1, np.int32), sh_nprim=np.ones(1, np.int32), sh_off=np.zeros(1, np.int32),
+                    exps=np.array([0.9]), coefs=np.ones(1), omega=0.4, n_occ=1, seed=1)
+    S = oracle_mod.overlap(wl)
+    P = np.array([[1.0 / S[0, 0]]])
+    ref = oracle_mod.jk(wl, P)
+    J, K, Sg, st = _gpu_jk(torch_cuda, wl, P)
+    assert abs(Sg[0, 0] - S[0, 0]) < 1e-13
+    assert abs(J[0, 0] - ref["J"][0, 0]) < TOL and abs(K[0, 0] - ref["K"][0, 0]) < TOL
+    assert abs(J[0, 0] - K[0, 0]) < TOL          # one function: (mm|mm) both ways
