@@ -43,7 +43,11 @@ __device__ __forceinline__ float ldg_volatile(const float *p)
 // memory (1320 B at L = 8: one CTA per SM).
 __host__ __device__ constexpr int k_nthreads(int) { return 128; }
 #define K_MIXED_LMAX 4                                        // highest class order with a mixed-precision kernel
-constexpr int KQ = 64;                                       // ring capacity per warp (power of two)
+constexpr int KQ = 64;                                       // ring capacity per warp (power of two), classes with L <= 4
+// Classes with L >= 5 evaluate in lockstep rounds in which the FOUR rings of the CTA are drained as one queue (see the
+// kernel): a warp may then collect up to 128 survivors before a round (enough to feed a whole round alone), so its ring holds up to 159
+__host__ __device__ constexpr int k_ring(int L) { return L >= 5 ? 256 : KQ; }
+__host__ __device__ constexpr int k_qstop(int L) { return L >= 5 ? 128 : 32; }
 constexpr int NIMG_K = 128;                                  // lattice images per CTA-level list chunk
 
 
@@ -52,7 +56,7 @@ constexpr size_t k_smem_bytes()
 {
     constexpr int L = LA + LB + LC + LD, NT = k_nthreads(L), NW = NT / 32;
     size_t d = (L > 4 ? (size_t)nherm(L) * NT : 0) + (size_t)NW * ncart(LA) * ncart(LD) + 3 * NIMG_K;
-    return d * sizeof(double) + 3 * NIMG_K * sizeof(float) + (size_t)NW * KQ * sizeof(int2) * (MIXED ? 2 : 1);
+    return d * sizeof(double) + 3 * NIMG_K * sizeof(float) + (size_t)NW * k_ring(L) * sizeof(int2) * (MIXED ? 2 : 1);
 }
 
 // light classes: at most 128 registers (L <= 3: 4 CTAs, 16 warps per SM) or 168 (L = 4: 3 CTAs); the few spilled
@@ -81,6 +85,8 @@ sr_k_kernel(SRParams p, const int2 *__restrict__ blocks, int nblocks)
     constexpr int NA = ncart(LA), ND = ncart(LD);
     constexpr bool RSMEM = L > 4;
     constexpr bool LOCKSTEP = L >= 5;
+    constexpr int KQ = k_ring(L), QSTOP = k_qstop(L);                 // shadows the namespace constant
+    static_assert(!(LOCKSTEP && MIXED), "the mixed mode exists for L <= 4 only");
     using Ev = KEval<LA, LB, LC, LD>;
     static_assert(Ev::NBRA == bra_terms<LA, LB>(), "generator and kernel disagree on the bra table");
     extern __shared__ __align__(16) double smem[];
@@ -93,6 +99,8 @@ sr_k_kernel(SRParams p, const int2 *__restrict__ blocks, int nblocks)
     int2 *queue = reinterpret_cast<int2 *>(sC + 3 * NIMG_K);          // [NW][KQ] (bra | ket << 16, image)
     int2 *queue32 = queue + NW * KQ;                                  // [NW][KQ] fp32 ring (MIXED)
     __shared__ int s_ctl[2];
+    __shared__ int s_cnt[4], s_head[4], s_done[4];                    // LOCKSTEP: the rings of the four warps, published per round
+    int2 *const qall = queue;
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     queue += w * KQ;
     queue32 += w * KQ;
@@ -178,7 +186,7 @@ sr_k_kernel(SRParams p, const int2 *__restrict__ blocks, int nblocks)
         float c_Dx = 0.f, c_Dy = 0.f, c_Dz = 0.f, c_thr = 0.f, c_ipi = 0.f;
         for (;;) {
             // ---- screen until 32 survivors are queued (in either ring) or the items run out ----
-            while (qn < 32 && (!MIXED || qn32 < 32)) {
+            while (qn < QSTOP && (!MIXED || qn32 < 32)) {
                 if (!have) {
                     if (imask == 0) {
                         if (ebase >= nitems) { items_done = true; break; }
@@ -252,47 +260,72 @@ sr_k_kernel(SRParams p, const int2 *__restrict__ blocks, int nblocks)
             }
             // a partly filled ring is evaluated only when this chunk's items are exhausted (its image indices
             // refer to the current list)
-            const bool w64 = qn >= 32 || (items_done && qn > 0);
-            const bool w32 = MIXED && (qn32 >= 32 || (items_done && qn32 > 0));
-            if (LOCKSTEP) {
-                // the evaluators of the high classes are 10-60 thousand instructions of straight-line code, far more
-                // than the instruction caches hold; the warps of a CTA therefore enter the evaluator together and
-                // share the fetched lines.  Every warp passes these barriers once per round until no warp has
-                // anything to evaluate.
-                const int any64 = __syncthreads_or(w64);
-                const int any32 = MIXED ? __syncthreads_or(w32) : 0;
-                if (!any64 && !any32) break;
-            } else if (!w64 && !w32) break;
-            // ---- evaluation: one primitive quartet-image per lane, oldest survivors first ----
-            if (w64) {
-                const int take = qn < 32 ? qn : 32;
-                int i = b0, j = k0, t = 0;
-                if (lane < take) {
-                    const int2 e = queue[(head + lane) & (KQ - 1)];
+            bool act = false, w32 = false;
+            int i = b0, j = k0, t = 0, consumed = 0;
+            if constexpr (LOCKSTEP) {
+                // The evaluators of the high classes are 10-60 thousand instructions of straight-line code, far more than
+                // the instruction caches hold: the warps of a CTA enter the evaluator together and share the fetched lines.
+                // A class of this kind holds only a few passes of quartets per warp, unevenly spread, so the four rings are
+                // drained as ONE queue (ring of warp 0 first, then 1, ...): thread g of the CTA takes entry g of that queue,
+                // whichever warp screened it -- every round runs with up to 128 busy lanes until all rings are empty.  (ncu
+                // on (dd|dp) before this: 39 % of the stall samples at the round barrier, 18 active lanes per instruction.)
+                if (lane == 0) { s_cnt[w] = qn; s_head[w] = head; s_done[w] = items_done ? 1 : 0; }
+                __syncthreads();
+                const int c0 = s_cnt[0], c1 = s_cnt[1], c2 = s_cnt[2], c3 = s_cnt[3];
+                const int tot = c0 + c1 + c2 + c3;
+                const bool alldone = (s_done[0] & s_done[1] & s_done[2] & s_done[3]) != 0;
+                const int take = tot < NT ? tot : NT;
+                const int g = threadIdx.x;
+                act = g < take;
+                if (act) {
+                    const int p1 = c0, p2 = c0 + c1, p3 = p2 + c2;
+                    const int sw = (g >= p1) + (g >= p2) + (g >= p3);
+                    const int li = g - (sw == 0 ? 0 : (sw == 1 ? p1 : (sw == 2 ? p2 : p3)));
+                    const int2 e = qall[sw * KQ + ((s_head[sw] + li) & (KQ - 1))];
                     i = b0 + (e.x & 0xffff); j = k0 + (int)((unsigned)e.x >> 16); t = e.y;
                 }
-                const long long eo = __ldg(K.eoff + i);
-                const double *__restrict__ bE = K.etab + eo;
-                if (lane < take) {
-                    const double X = __ldg(K.Px + j) + sT[t] - __ldg(K.Px + i), Y = __ldg(K.Py + j) + sT[NIMG_K + t] - __ldg(K.Py + i),
-                                 Z = __ldg(K.Pz + j) + sT[2 * NIMG_K + t] - __ldg(K.Pz + i);
-                    const double pb = __ldg(K.p + i), q = __ldg(K.p + j);
-                    const double r2 = X * X + Y * Y + Z * Z;
-                    const double s = rsqrt(pb + q);
-                    const double alpha = pb * q * s * s;
-                    const double th = lat.omega * rsqrt(alpha + lat.omega2);
-                    const double alpha_w = alpha * th * th;
-                    const double pref = r2 <= p.rcut2 ? __ldg(K.coef + i) * __ldg(K.coef + j) * s : 0.0;
-                    const double *__restrict__ Pb = p.Pp + (size_t)__ldg(K.aoB + i) * p.ldP + __ldg(K.aoB + j);
-                    double Rm[L + 1];
-                    boys_merged<L, double>(p.boys, r2, alpha, alpha_w, th, pref, Rm);
-                    Ev::template run<32, double>(bE, K.etab + __ldg(K.eoff + j), Pb, p.ldP, Rm, X, Y, Z, Rs, Kacc);
+                const int before = w == 0 ? 0 : (w == 1 ? c0 : (w == 2 ? c0 + c1 : c0 + c1 + c2));
+                consumed = take - before;                              // entries of this warp's ring taken by the round
+                consumed = consumed < 0 ? 0 : (consumed > qn ? qn : consumed);
+                __syncthreads();                                       // counters and entries are read: the owners may push again
+                if (tot == 0) {
+                    if (alldone) break;
+                    continue;
                 }
-                head = (head + take) & (KQ - 1);
-                qn -= take;
-                nquart += take;
-                __syncwarp();
+            } else {
+                const bool w64 = qn >= 32 || (items_done && qn > 0);
+                w32 = MIXED && (qn32 >= 32 || (items_done && qn32 > 0));
+                if (!w64 && !w32) break;
+                if (w64) {
+                    consumed = qn < 32 ? qn : 32;
+                    act = lane < consumed;
+                    if (act) {
+                        const int2 e = queue[(head + lane) & (KQ - 1)];
+                        i = b0 + (e.x & 0xffff); j = k0 + (int)((unsigned)e.x >> 16); t = e.y;
+                    }
+                }
             }
+            // ---- evaluation: one primitive quartet-image per lane, oldest survivors first ----
+            if (act) {
+                const double *__restrict__ bE = K.etab + __ldg(K.eoff + i);
+                const double X = __ldg(K.Px + j) + sT[t] - __ldg(K.Px + i), Y = __ldg(K.Py + j) + sT[NIMG_K + t] - __ldg(K.Py + i),
+                             Z = __ldg(K.Pz + j) + sT[2 * NIMG_K + t] - __ldg(K.Pz + i);
+                const double pb = __ldg(K.p + i), q = __ldg(K.p + j);
+                const double r2 = X * X + Y * Y + Z * Z;
+                const double s = rsqrt(pb + q);
+                const double alpha = pb * q * s * s;
+                const double th = lat.omega * rsqrt(alpha + lat.omega2);
+                const double alpha_w = alpha * th * th;
+                const double pref = r2 <= p.rcut2 ? __ldg(K.coef + i) * __ldg(K.coef + j) * s : 0.0;
+                const double *__restrict__ Pb = p.Pp + (size_t)__ldg(K.aoB + i) * p.ldP + __ldg(K.aoB + j);
+                double Rm[L + 1];
+                boys_merged<L, double>(p.boys, r2, alpha, alpha_w, th, pref, Rm);
+                Ev::template run<32, double>(bE, K.etab + __ldg(K.eoff + j), Pb, p.ldP, Rm, X, Y, Z, Rs, Kacc);
+            }
+            head = (head + consumed) & (KQ - 1);
+            qn -= consumed;
+            nquart += consumed;
+            __syncwarp();
             if constexpr (MIXED) if (w32) {
                 const int take = qn32 < 32 ? qn32 : 32;
                 int i = b0, j = k0, t = 0;
