@@ -41,13 +41,18 @@ __device__ __forceinline__ float ldg_volatile(const float *p)
 // CTA size: 128 threads in every class.  The warps of a CTA enter the evaluator in lockstep at L >= 5 (see LOCKSTEP
 // below), so four warps share the instruction fetches; the R column of a thread takes 8*nherm(L) bytes of shared
 // memory (1320 B at L = 8: one CTA per SM).
+// (256-thread CTAs at L = 5, 6 -- 8 warps per lockstep round -- measured 86 / 48 ms against 70 / 47 ms with 128)
 __host__ __device__ constexpr int k_nthreads(int) { return 128; }
 #define K_MIXED_LMAX 4                                        // highest class order with a mixed-precision kernel
+#ifndef K_LOCK_LMIN
+#define K_LOCK_LMIN 5                                         // lowest class order evaluated in lockstep rounds (fp64 kernels; at 4: 70 -> 84 ms)
+#endif
 constexpr int KQ = 64;                                       // ring capacity per warp (power of two), classes with L <= 4
 // Classes with L >= 5 evaluate in lockstep rounds in which the FOUR rings of the CTA are drained as one queue (see the
 // kernel): a warp may then collect up to 128 survivors before a round (enough to feed a whole round alone), so its ring holds up to 159
-__host__ __device__ constexpr int k_ring(int L) { return L >= 5 ? 256 : KQ; }
-__host__ __device__ constexpr int k_qstop(int L) { return L >= 5 ? 128 : 32; }
+__host__ __device__ constexpr bool k_lockstep(int L, bool mixed) { return L >= K_LOCK_LMIN && !mixed; }
+__host__ __device__ constexpr int k_ring(int L, bool mixed) { return k_lockstep(L, mixed) ? 256 : KQ; }
+__host__ __device__ constexpr int k_qstop(int L, bool mixed) { return k_lockstep(L, mixed) ? 128 : 32; }
 constexpr int NIMG_K = 128;                                  // lattice images per CTA-level list chunk
 
 
@@ -56,7 +61,7 @@ constexpr size_t k_smem_bytes()
 {
     constexpr int L = LA + LB + LC + LD, NT = k_nthreads(L), NW = NT / 32;
     size_t d = (L > 4 ? (size_t)nherm(L) * NT : 0) + (size_t)NW * ncart(LA) * ncart(LD) + 3 * NIMG_K;
-    return d * sizeof(double) + 3 * NIMG_K * sizeof(float) + (size_t)NW * k_ring(L) * sizeof(int2) * (MIXED ? 2 : 1);
+    return d * sizeof(double) + 3 * NIMG_K * sizeof(float) + (size_t)NW * k_ring(L, MIXED) * sizeof(int2) * (MIXED ? 2 : 1);
 }
 
 // light classes: at most 128 registers (L <= 3: 4 CTAs, 16 warps per SM) or 168 (L = 4: 3 CTAs); the few spilled
@@ -84,8 +89,8 @@ sr_k_kernel(SRParams p, const int2 *__restrict__ blocks, int nblocks)
     constexpr int NT = k_nthreads(L), NW = NT / 32;
     constexpr int NA = ncart(LA), ND = ncart(LD);
     constexpr bool RSMEM = L > 4;
-    constexpr bool LOCKSTEP = L >= 5;
-    constexpr int KQ = k_ring(L), QSTOP = k_qstop(L);                 // shadows the namespace constant
+    constexpr bool LOCKSTEP = k_lockstep(L, MIXED);
+    constexpr int KQ = k_ring(L, MIXED), QSTOP = k_qstop(L, MIXED);                 // shadows the namespace constant
     static_assert(!(LOCKSTEP && MIXED), "the mixed mode exists for L <= 4 only");
     using Ev = KEval<LA, LB, LC, LD>;
     static_assert(Ev::NBRA == bra_terms<LA, LB>(), "generator and kernel disagree on the bra table");
@@ -99,7 +104,7 @@ sr_k_kernel(SRParams p, const int2 *__restrict__ blocks, int nblocks)
     int2 *queue = reinterpret_cast<int2 *>(sC + 3 * NIMG_K);          // [NW][KQ] (bra | ket << 16, image)
     int2 *queue32 = queue + NW * KQ;                                  // [NW][KQ] fp32 ring (MIXED)
     __shared__ int s_ctl[2];
-    __shared__ int s_cnt[4], s_head[4], s_done[4];                    // LOCKSTEP: the rings of the four warps, published per round
+    __shared__ int s_cnt[8], s_head[8], s_done[8];                    // LOCKSTEP: the rings of the four warps, published per round
     int2 *const qall = queue;
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     queue += w * KQ;
@@ -271,20 +276,26 @@ sr_k_kernel(SRParams p, const int2 *__restrict__ blocks, int nblocks)
                 // on (dd|dp) before this: 39 % of the stall samples at the round barrier, 18 active lanes per instruction.)
                 if (lane == 0) { s_cnt[w] = qn; s_head[w] = head; s_done[w] = items_done ? 1 : 0; }
                 __syncthreads();
-                const int c0 = s_cnt[0], c1 = s_cnt[1], c2 = s_cnt[2], c3 = s_cnt[3];
-                const int tot = c0 + c1 + c2 + c3;
-                const bool alldone = (s_done[0] & s_done[1] & s_done[2] & s_done[3]) != 0;
+                int cnt[NW], tot = 0, before = 0;
+                bool alldone = true;
+#pragma unroll
+                for (int x = 0; x < NW; ++x) {
+                    cnt[x] = s_cnt[x];
+                    if (x < w) before += cnt[x];
+                    tot += cnt[x];
+                    alldone = alldone && s_done[x] != 0;
+                }
                 const int take = tot < NT ? tot : NT;
                 const int g = threadIdx.x;
                 act = g < take;
                 if (act) {
-                    const int p1 = c0, p2 = c0 + c1, p3 = p2 + c2;
-                    const int sw = (g >= p1) + (g >= p2) + (g >= p3);
-                    const int li = g - (sw == 0 ? 0 : (sw == 1 ? p1 : (sw == 2 ? p2 : p3)));
-                    const int2 e = qall[sw * KQ + ((s_head[sw] + li) & (KQ - 1))];
+                    int sw = 0, base = 0;
+#pragma unroll
+                    for (int x = 0; x < NW - 1; ++x)
+                        if (sw == x && g >= base + cnt[x]) { base += cnt[x]; ++sw; }
+                    const int2 e = qall[sw * KQ + ((s_head[sw] + (g - base)) & (KQ - 1))];
                     i = b0 + (e.x & 0xffff); j = k0 + (int)((unsigned)e.x >> 16); t = e.y;
                 }
-                const int before = w == 0 ? 0 : (w == 1 ? c0 : (w == 2 ? c0 + c1 : c0 + c1 + c2));
                 consumed = take - before;                              // entries of this warp's ring taken by the round
                 consumed = consumed < 0 ? 0 : (consumed > qn ? qn : consumed);
                 __syncthreads();                                       // counters and entries are read: the owners may push again
