@@ -158,7 +158,8 @@ def _ncu_traffic(kernel):
 def h_nb(st, n):
     """G vectors per reciprocal-space batch as pbc_jk_create sizes them (stacks <= 12 GB, at most 64)"""
     np_ = ((n + 63) // 64) * 64
-    return max(1, min(64, int(12.0e9 // (np_ * np_ * 16)), max(st["n_g"], 1)))
+    nb = max(1, min(64, int(12.0e9 // (np_ * np_ * 16)), max(st["n_g"], 1)))
+    return (nb // 16) * 16 if nb >= 16 else nb
 
 
 def _oracle_sample_blocks(wl, nblk, seed=12345):

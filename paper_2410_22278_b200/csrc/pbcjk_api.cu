@@ -711,8 +711,11 @@ int setup(pbc_jk *h, const pbc_cell *cell, const pbc_atoms *atoms, const pbc_she
         // G batch: A' and Y stacks of Np x 2nb x Np doubles each, at most 12 GB per stack (180 GB HBM3e per GPU)
         int nb = cut.lr_g_batch > 0 ? cut.lr_g_batch : (int)std::min<double>(64.0, std::floor(12.0e9 / (double)(Np * Np * 16)));
         nb = std::max(1, std::min(std::min(nb, 64), std::max(h->nG, 1)));      // the slot kernels hold at most 128 slots
+        // the slot count of a batch is rounded up to the GEMM k-tile (32); padded slots are pure waste in both GEMMs, so the
+        // default batch holds a multiple of 16 G vectors (2 slots each)
+        if (cut.lr_g_batch <= 0 && nb >= 16) nb = (nb / 16) * 16;
         h->nb = nb;
-        h->Smax = ((2 * nb + 15) / 16) * 16;             // slots of a full batch (multiple of 16)
+        h->Smax = ((2 * nb + 31) / 32) * 32;             // slots of a full batch (multiple of 32)
         h->ld = (size_t)h->Smax * Np;
         // split of the K^LR accumulation over the rows of the factor: the lower 128x128 tiles times nsplit should
         // fill whole waves of one CTA per SM
@@ -1008,7 +1011,7 @@ static int build_impl(pbc_jk *h, const double *P, const double *Corb, int nocc, 
         int ibatch = 0;
         for (int g0 = 0; g0 < h->nG; g0 += h->nb, ++ibatch) {
             if (ibatch % h->shard_n != h->shard_rank) continue;      // multi-GPU: G batches dealt round-robin
-            const int nb = std::min(h->nb, h->nG - g0), S = ((2 * nb + 15) / 16) * 16;
+            const int nb = std::min(h->nb, h->nG - g0), S = ((2 * nb + 31) / 32) * 32;
             CK(set_layout(S));
             launch_agen(h->lr, g0, nb, S, 0.0, h->Astack, h->Pp, J ? h->rho : nullptr, st);
             nl += n_agen + (J ? 3 : 0) + (K ? 2 : 0);
@@ -1021,14 +1024,14 @@ static int build_impl(pbc_jk *h, const double *P, const double *Corb, int nocc, 
     }
     // ---- A9: the G = 0 slot, weight -pi/(Omega w^2), A = S ----
     if (doSELF) {
-        CK(set_layout(16));
-        launch_agen(h->lr, -1, 1, 16, std::sqrt(h->c0), h->Astack, h->Pp, J ? h->rho : nullptr, st);
+        CK(set_layout(32));
+        launch_agen(h->lr, -1, 1, 32, std::sqrt(h->c0), h->Astack, h->Pp, J ? h->rho : nullptr, st);
         nl += n_agen + (J ? 3 : 0) + (K ? 2 : 0);
         if (J) {
-            launch_rho_final(h->lr, 16, h->rho, st);
-            launch_jlr_accum(h->Astack, Np, N, 16, h->rho, -1.0, h->Jlr, st);
+            launch_rho_final(h->lr, 32, h->rho, st);
+            launch_jlr_accum(h->Astack, Np, N, 32, h->rho, -1.0, h->Jlr, st);
         }
-        if (K) klr_batch(16, -1.0, h->nsplit);
+        if (K) klr_batch(32, -1.0, h->nsplit);
     }
     CK(cudaEventRecord(h->ev[4], st));
     if (J && doSR && h->U.nsp > 0) {
@@ -1141,7 +1144,7 @@ int pbc_jk_one_electron(pbc_jk *h, const double *charges_host, double *T, double
             cudaMemsetAsync(h->Astack, 0, (size_t)Np * Np * S * sizeof(double), st);
         };
         for (int g0 = 0; g0 < h->nG; g0 += h->nb) {
-            const int nb = std::min(h->nb, h->nG - g0), S = ((2 * nb + 15) / 16) * 16;
+            const int nb = std::min(h->nb, h->nG - g0), S = ((2 * nb + 31) / 32) * 32;
             set_layout(S);
             launch_agen(h->lr, g0, nb, S, 0.0, h->Astack, nullptr, nullptr, st);
             launch_rho_nuc(h->lr, g0, nb, S, 0.0, dx, dq, na, h->rho, st);

@@ -426,8 +426,8 @@ void launch_jlr_accum(const double *Astack, int Np, int N, int S, const double *
 
 // ---------------------------------------------------------------- FP64 tensor-core GEMM (A8, A9)
 namespace {
-constexpr int BM = 128, BN = 128, BK = 16;
-constexpr int NSTAGE = 4;     // cp.async ring: tiles t+1 .. t+3 are in flight while tile t is multiplied, one barrier per tile
+constexpr int BM = 128, BN = 128, BK = 32;
+constexpr int NSTAGE = 3;     // cp.async ring: tiles t+1, t+2 are in flight while tile t is multiplied, one barrier per tile
                               // (the kernel holds 166 registers x 256 threads: one CTA per SM, so nothing else hides the waits)
 constexpr int SA = BK + 4;    // row stride of the A tile [m][k]: (lane/4)*20 + lane%4 hits every bank pair twice
 constexpr int SB = BN + 8;    // row stride of the B tile [k][n]: (lane%4)*136 + lane/4 likewise
@@ -501,7 +501,7 @@ __global__ void __launch_bounds__(256) dgemm_kernel(int Kb, int nbatch, double a
             const double *Ab = A + (size_t)b * strideA + (size_t)(bm * BM) * lda + k0;
 #pragma unroll
             for (int c = tid; c < BM * BK / 2; c += 256) {
-                const int row = c >> 3, c2 = c & 7;
+                const int row = c / (BK / 2), c2 = c % (BK / 2);
                 cp_async16(as + row * SA + c2 * 2, Ab + (size_t)row * lda + c2 * 2);
             }
         }
@@ -509,7 +509,7 @@ __global__ void __launch_bounds__(256) dgemm_kernel(int Kb, int nbatch, double a
             const double *Bb = B + (size_t)b * strideB + (size_t)(bn * BN) * ldb + k0;
 #pragma unroll
             for (int c = tid; c < BN * BK / 2; c += 256) {
-                const int row = c >> 3, c2 = c & 7;
+                const int row = c / (BK / 2), c2 = c % (BK / 2);
                 cp_async16(bs + row * SA + c2 * 2, Bb + (size_t)row * ldb + c2 * 2);
             }
         } else {
