@@ -49,10 +49,11 @@ __host__ __device__ constexpr int k_nthreads(int) { return 128; }
 #endif
 constexpr int KQ = 64;                                       // ring capacity per warp (power of two), classes with L <= 4
 // Classes with L >= 5 evaluate in lockstep rounds in which the FOUR rings of the CTA are drained as one queue (see the
-// kernel): a warp may then collect up to 128 survivors before a round (enough to feed a whole round alone), so its ring holds up to 159
+// kernel): a warp may then collect up to 64 survivors before a round, so its ring holds up to 95 (128 / ring 256 measured:
+// water64 K 366.6 -> 363.3 ms but si64 K 1868 -> 1977 ms; 32: 392 and 1956 ms)
 __host__ __device__ constexpr bool k_lockstep(int L, bool mixed) { return L >= K_LOCK_LMIN && !mixed; }
-__host__ __device__ constexpr int k_ring(int L, bool mixed) { return k_lockstep(L, mixed) ? 256 : KQ; }
-__host__ __device__ constexpr int k_qstop(int L, bool mixed) { return k_lockstep(L, mixed) ? 128 : 32; }
+__host__ __device__ constexpr int k_ring(int L, bool mixed) { return k_lockstep(L, mixed) ? 128 : KQ; }
+__host__ __device__ constexpr int k_qstop(int L, bool mixed) { return k_lockstep(L, mixed) ? 64 : 32; }
 constexpr int NIMG_K = 128;                                  // lattice images per CTA-level list chunk
 
 
