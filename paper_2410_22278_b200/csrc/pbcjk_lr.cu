@@ -487,54 +487,62 @@ __global__ void __launch_bounds__(256) dgemm_kernel(int Kb, int nbatch, double a
 #pragma unroll
         for (int j = 0; j < 4; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
 
-    auto load_tile = [&](int t, int buf) {
-        const int b = bat0 + t / kt_per, k0 = (t % kt_per) * BK;
-        double *as = As + buf * A_TILE, *bs = Bs + buf * B_TILE;
-        if (TA) {
-            const double *Ab = A + (size_t)b * strideA + (size_t)k0 * lda + bm * BM;
-#pragma unroll
-            for (int c = tid; c < BK * BM / 2; c += 256) {
-                const int row = c >> 6, c2 = c & 63;
-                cp_async16(as + row * SB + c2 * 2, Ab + (size_t)row * lda + c2 * 2);
-            }
-        } else {
-            const double *Ab = A + (size_t)b * strideA + (size_t)(bm * BM) * lda + k0;
-#pragma unroll
-            for (int c = tid; c < BM * BK / 2; c += 256) {
-                const int row = c / (BK / 2), c2 = c % (BK / 2);
-                cp_async16(as + row * SA + c2 * 2, Ab + (size_t)row * lda + c2 * 2);
-            }
-        }
-        if (TB) {
-            const double *Bb = B + (size_t)b * strideB + (size_t)(bn * BN) * ldb + k0;
-#pragma unroll
-            for (int c = tid; c < BN * BK / 2; c += 256) {
-                const int row = c / (BK / 2), c2 = c % (BK / 2);
-                cp_async16(bs + row * SA + c2 * 2, Bb + (size_t)row * ldb + c2 * 2);
-            }
-        } else {
-            const double *Bb = B + (size_t)b * strideB + (size_t)k0 * ldb + bn * BN;
-#pragma unroll
-            for (int c = tid; c < BK * BN / 2; c += 256) {
-                const int row = c >> 6, c2 = c & 63;
-                cp_async16(bs + row * SB + c2 * 2, Bb + (size_t)row * ldb + c2 * 2);
-            }
-        }
+    // Each thread copies 8 + 8 16-byte pieces per k-tile.  Their global addresses are one per-thread base pointer per operand
+    // plus a multiple of a fixed stride, and the (batch, k) position of the next tile to fetch advances incrementally -- the
+    // tiles are requested in order -- so that issuing a tile costs a few instructions per cp.async (the 64-bit index
+    // arithmetic per piece, and a division per tile, took the DMMA warps of both schedulers off the pipe after every barrier).
+    const double *gA, *gB;
+    size_t stepA, stepB, kstepA, kstepB;
+    int soffA, soffB;                                      // element offsets of this thread's first piece inside a stage
+    if (TA) {
+        gA = A + (size_t)bat0 * strideA + (size_t)(tid >> 6) * lda + bm * BM + (tid & 63) * 2;
+        stepA = 4 * lda; kstepA = (size_t)BK * lda; soffA = (tid >> 6) * SB + (tid & 63) * 2;
+    } else {
+        gA = A + (size_t)bat0 * strideA + (size_t)(bm * BM + (tid >> 4)) * lda + (tid & 15) * 2;
+        stepA = 16 * lda; kstepA = BK; soffA = (tid >> 4) * SA + (tid & 15) * 2;
+    }
+    if (TB) {
+        gB = B + (size_t)bat0 * strideB + (size_t)(bn * BN + (tid >> 4)) * ldb + (tid & 15) * 2;
+        stepB = 16 * ldb; kstepB = BK; soffB = (tid >> 4) * SA + (tid & 15) * 2;
+    } else {
+        gB = B + (size_t)bat0 * strideB + (size_t)(tid >> 6) * ldb + bn * BN + (tid & 63) * 2;
+        stepB = 4 * ldb; kstepB = (size_t)BK * ldb; soffB = (tid >> 6) * SB + (tid & 63) * 2;
+    }
+    static_assert(BK == 32 && BM == 128 && BN == 128, "piece mapping of load_tile");
+    int ld_kt = 0;                                          // k-tile of the next fetch inside its batch
+    auto load_piece = [&](int buf, int i) {                 // piece i (0..7) of the A and of the B tile
+        cp_async16(As + buf * A_TILE + soffA + i * (TA ? 4 * SB : 16 * SA), gA + i * stepA);
+        cp_async16(Bs + buf * B_TILE + soffB + i * (TB ? 16 * SA : 4 * SB), gB + i * stepB);
+    };
+    auto load_advance = [&]() {
         asm volatile("cp.async.commit_group;\n" ::);
+        if (++ld_kt == kt_per) {                            // next batch: back to k = 0
+            ld_kt = 0;
+            gA += strideA - (size_t)(kt_per - 1) * kstepA;
+            gB += strideB - (size_t)(kt_per - 1) * kstepB;
+        } else {
+            gA += kstepA;
+            gB += kstepB;
+        }
     };
 
     // prologue: NSTAGE - 1 tiles in flight (empty commit groups keep the group count uniform)
 #pragma unroll
     for (int t = 0; t < NSTAGE - 1; ++t) {
-        if (t < ntile) load_tile(t, t);
+        if (t < ntile) {
+#pragma unroll
+            for (int i = 0; i < 8; ++i) load_piece(t, i);
+            load_advance();
+        }
         else asm volatile("cp.async.commit_group;\n" ::);
     }
     for (int t = 0; t < ntile; ++t) {
         const int buf = t % NSTAGE;
         asm volatile("cp.async.wait_group %0;\n" ::"n"(NSTAGE - 2));       // tile t has landed (for this thread)
         __syncthreads();                                                    // ... for all; and everyone is done with tile t-1
-        if (t + NSTAGE - 1 < ntile) load_tile(t + NSTAGE - 1, (t + NSTAGE - 1) % NSTAGE);   // into the buffer of tile t-1
-        else asm volatile("cp.async.commit_group;\n" ::);
+        // tile t + NSTAGE - 1 goes into the buffer of tile t-1: one A and one B piece per k-step, between the DMMAs
+        const bool fetch = t + NSTAGE - 1 < ntile;
+        const int fbuf = (t + NSTAGE - 1) % NSTAGE;
         const double *as = TA ? As + buf * A_TILE + (lane & 3) * SB + wm * 64 + (lane >> 2)
                               : As + buf * A_TILE + (wm * 64 + (lane >> 2)) * SA + (lane & 3);
         const double *bs = TB ? Bs + buf * B_TILE + (wn * 32 + (lane >> 2)) * SA + (lane & 3)
@@ -546,11 +554,14 @@ __global__ void __launch_bounds__(256) dgemm_kernel(int Kb, int nbatch, double a
             for (int i = 0; i < 8; ++i) a[i] = TA ? as[kk * SB + i * 8] : as[i * 8 * SA + kk];
 #pragma unroll
             for (int j = 0; j < 4; ++j) b[j] = TB ? bs[j * 8 * SA + kk] : bs[kk * SB + j * 8];
+            if (fetch) load_piece(fbuf, kk >> 2);
 #pragma unroll
             for (int i = 0; i < 8; ++i)
 #pragma unroll
                 for (int j = 0; j < 4; ++j) dmma(acc[i][j][0], acc[i][j][1], a[i], b[j]);
         }
+        if (fetch) load_advance();
+        else asm volatile("cp.async.commit_group;\n" ::);
     }
 #pragma unroll
     for (int i = 0; i < 8; ++i)
