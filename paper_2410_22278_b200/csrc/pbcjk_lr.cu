@@ -397,7 +397,9 @@ void launch_rho_final(const LRParams &p, int S, double *rho, cudaStream_t st)
     rho_stage2_kernel<<<1, 128, 0, st>>>(rho + S, S, rho);
 }
 
-// Jacc[m][n] += sign * sum_slot A'[m][n][slot] rho'[slot]: one warp per matrix element, lanes over the slots
+// Jacc[m][n] += sign * sum_slot A'[m][n][slot] rho'[slot]: one warp per matrix element, lanes over the slots.
+// A'[m][n][.] and A'[n][m][.] hold the same bits (agen_kernel stores one value at both places), so only n <= m is read
+// -- half of the batch -- and the sum goes to both elements.
 __global__ void __launch_bounds__(256) jlr_accum_kernel(const double *__restrict__ Astack, size_t ld, int N, int S,
                                                         const double *__restrict__ rho, double sign, double *__restrict__ Jacc)
 {
@@ -406,7 +408,7 @@ __global__ void __launch_bounds__(256) jlr_accum_kernel(const double *__restrict
     double r[4];
 #pragma unroll
     for (int k = 0; k < 4; ++k) r[k] = lane + 32 * k < S ? rho[lane + 32 * k] : 0.0;
-    for (int n = blockIdx.x * 8 + w; n < N; n += gridDim.x * 8) {
+    for (int n = blockIdx.x * 8 + w; n <= m; n += gridDim.x * 8) {
         const double *a = Astack + (size_t)m * ld + (size_t)n * S;
         double acc = 0.0;
 #pragma unroll
@@ -414,7 +416,10 @@ __global__ void __launch_bounds__(256) jlr_accum_kernel(const double *__restrict
             if (lane + 32 * k < S) acc = fma(a[lane + 32 * k], r[k], acc);
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
-        if (lane == 0) Jacc[(size_t)m * N + n] += sign * acc;
+        if (lane == 0) {
+            Jacc[(size_t)m * N + n] += sign * acc;
+            if (n != m) Jacc[(size_t)n * N + m] += sign * acc;
+        }
     }
 }
 void launch_jlr_accum(const double *Astack, int Np, int N, int S, const double *rho, double sign, double *Jacc, cudaStream_t st)
