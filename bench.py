@@ -442,6 +442,11 @@ def main():
                    "frac": gemm_tf / pk["fp64_dmma"] if pk["fp64_dmma"] > 0 else 0.0, "share_of_step": gemm_ms / ms_per_step,
                    "peak_kind": f"FP64 tensor (DMMA) micro-benchmark on this box; derived from MEASURED_PEAKS bf16 x 45/2250: "
                                 f"{dmma_derived:.1f} TFLOP/s ({peaks_kind})",
+                   # context for the fraction: DMMA and DFMA warps side by side (sum of both rates: one shared
+                   # FP64 pipe if it equals the peak) and the kernel's inner loop without its global loads
+                   "fp64_probes_tflops": {"dmma": round(pk["fp64_dmma"], 2), "dfma": round(pk["fp64_fma"], 2),
+                                          "dmma_and_dfma_side_by_side": round(pk["fp64_mixed_pipe"], 2),
+                                          "gemm_inner_loop_no_global_loads": round(pk["fp64_dmma_loop"], 2)},
                    "flop_per_launch_pair": gemm_flop / max(1, n_gemm_launch // 2), "rank_of_P": r_p, "g_slots": slots,
                    "ms_per_launch_pair": gemm_ms / max(1, n_gemm_launch // 2),
                    "traffic": _ncu_traffic("dgemm_kernel<0,0>"),

@@ -315,12 +315,14 @@ PEAKS_LIB_PATH = os.path.join(_HERE, "libpbc_jk_benchpeaks.so")
 
 def bench_peaks(iters: int = 20000) -> dict:
     """bench.py's roofline denominators measured on the current device (helper library outside the product ABI):
-    FP64 FMA, FP32 FMA and FP64 tensor-core (DMMA) TFLOP/s."""
+    FP64 FMA, FP32 FMA and FP64 tensor-core (DMMA) TFLOP/s; `fp64_mixed_pipe` = DMMA and DFMA warps side by side (sum of
+    both rates: equal to the single peaks when the two share a pipe), `fp64_dmma_loop` = the GEMM's inner loop (shared-memory
+    fragment loads + DMMA + barrier) without its global loads."""
     if not os.path.exists(PEAKS_LIB_PATH):
         raise RuntimeError(f"{PEAKS_LIB_PATH} is missing: build it with `python -m paper_2410_22278_b200.build`")
     lib = C.CDLL(PEAKS_LIB_PATH)
     out = {}
-    for name in ("fp64_fma", "fp32_fma", "fp64_dmma"):
+    for name in ("fp64_fma", "fp32_fma", "fp64_dmma", "fp64_mixed_pipe", "fp64_dmma_loop"):
         f = getattr(lib, f"bench_{name}_peak")
         f.argtypes = [C.c_int32, C.POINTER(C.c_double)]
         f.restype = C.c_int

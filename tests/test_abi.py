@@ -88,3 +88,19 @@ def test_product_does_not_import_oracle():
             txt = open(os.path.join(ROOT, "oracle", f)).read()
             assert "paper_2410_22278_b200 import" not in txt and "import paper_2410_22278_b200" not in txt, f
             assert "libpbc_jk.so" not in txt
+
+
+def test_bench_peaks_helper_exports_and_refuses_without_gpu(lib):
+    """bench.py's measurement helper (outside the product ABI) exports its five probes; without a device each fails."""
+    from paper_2410_22278_b200 import binding
+    hl = C.CDLL(binding.PEAKS_LIB_PATH)
+    for name in ("fp64_fma", "fp32_fma", "fp64_dmma", "fp64_mixed_pipe", "fp64_dmma_loop"):
+        f = getattr(hl, f"bench_{name}_peak")
+        f.argtypes = [C.c_int32, C.POINTER(C.c_double)]
+        f.restype = C.c_int
+        import torch
+        if not torch.cuda.is_available():
+            v = C.c_double(-7.0)
+            assert f(10, C.byref(v)) != 0 and v.value == -7.0
+    # the product library holds none of them
+    assert not hasattr(lib, "bench_fp64_dmma_peak")
