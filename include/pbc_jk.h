@@ -126,6 +126,21 @@ int pbc_jk_nbf(const pbc_jk *h);
 int pbc_jk_overlap(const pbc_jk *h, double *S_host);
 
 /*
+ * Allocation-free variant for callers that cannot call cudaMalloc (CUDA graph capture, tight serving loops, harnesses
+ * that forbid it): recomputes the crystalline overlap S (eq 21, S_mn = rho_mn(G = 0), the same kernels
+ * pbc_jk_create runs) into `S_dev`, N*N doubles row-major, DEVICE memory, caller-owned, overwritten.  All work is
+ * enqueued on `cuda_stream`; the call allocates nothing (no cudaMalloc/cudaFree, no allocating library routine) and
+ * does not synchronise the host.  Its scratch is a file-scope device array inside the library, sized for at most
+ * PBC_JK_NOALLOC_MAX_NBF basis functions after padding N to a multiple of 64 (4 MiB, held by every GPU that loads
+ * the library until the process exits); a larger handle is refused with PBC_JK_ERR_UNSUPPORTED and a text in
+ * pbc_jk_last_error.  ALL calls of the process share that array, on every handle and stream: calls that overlap on
+ * the GPU race -- order them on one stream or with events.  The array keeps the last call's contents; each call
+ * clears the part it reads before use.  Must be called with the handle's device current.
+ */
+#define PBC_JK_NOALLOC_MAX_NBF 512
+int pbc_jk_overlap_noalloc(pbc_jk *h, double *S_dev, void *cuda_stream);
+
+/*
  * A4-A10: one J+K build for density P (symmetric, N x N fp64 row-major, DEVICE).  J and/or K may
  * be NULL to skip that matrix; otherwise they are OVERWRITTEN with the full matrices (SR+LR+SELF).
  * All work is enqueued on `cuda_stream` (a cudaStream_t, NULL = default stream); the call does not

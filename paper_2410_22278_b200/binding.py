@@ -19,7 +19,7 @@ PBC_JK_OK = 0
 STATUS = {0: "OK", -1: "INVALID_ARG", -2: "NOMEM", -3: "CUDA", -4: "UNSUPPORTED"}
 
 # every symbol include/pbc_jk.h declares (checked by tests/test_abi.py)
-SYMBOLS = ["pbc_jk_create", "pbc_jk_nbf", "pbc_jk_overlap", "pbc_jk_build", "pbc_jk_build_orbitals", "pbc_jk_build_host",
+SYMBOLS = ["pbc_jk_create", "pbc_jk_nbf", "pbc_jk_overlap", "pbc_jk_overlap_noalloc", "pbc_jk_build", "pbc_jk_build_orbitals", "pbc_jk_build_host",
            "pbc_jk_one_electron", "pbc_jk_set_parts", "pbc_jk_set_shard", "pbc_jk_get_stats", "pbc_jk_set_profile", "pbc_jk_get_class_stats",
            "pbc_jk_last_error", "pbc_jk_destroy"]
 
@@ -77,6 +77,8 @@ def load() -> C.CDLL:
         lib.pbc_jk_nbf.restype = C.c_int
         lib.pbc_jk_overlap.argtypes = [C.c_void_p, C.c_void_p]
         lib.pbc_jk_overlap.restype = C.c_int
+        lib.pbc_jk_overlap_noalloc.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+        lib.pbc_jk_overlap_noalloc.restype = C.c_int
         lib.pbc_jk_build.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         lib.pbc_jk_build.restype = C.c_int
         lib.pbc_jk_build_orbitals.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p]
@@ -190,6 +192,19 @@ class PbcJK:
         S = np.zeros((self.nbf, self.nbf))
         self._check(load().pbc_jk_overlap(self._h, S.ctypes.data))
         return S
+
+    def overlap_noalloc(self, S_dev, stream=None):
+        """S into a caller's device tensor (N x N fp64, overwritten) through the entry point that allocates nothing: its
+        scratch is a static device array inside the library (N padded to 64 must not exceed PBC_JK_NOALLOC_MAX_NBF = 512).
+        Every call shares that array: calls that overlap on the GPU race."""
+        import torch
+
+        n = self.nbf
+        if not (S_dev.is_cuda and S_dev.dtype == torch.float64 and S_dev.is_contiguous() and tuple(S_dev.shape) == (n, n)):
+            raise ValueError("S_dev must be a contiguous float64 CUDA tensor of shape (nbf, nbf)")
+        st = torch.cuda.current_stream().cuda_stream if stream is None else int(stream)
+        self._check(load().pbc_jk_overlap_noalloc(self._h, S_dev.data_ptr(), st))
+        return S_dev
 
     def set_parts(self, parts: str = "sr+lr+self"):
         m = 0

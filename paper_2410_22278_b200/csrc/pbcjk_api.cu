@@ -86,6 +86,8 @@ struct pbc_jk {
     int shard_rank = 0, shard_n = 1;     // multi-GPU share of every build (pbc_jk_set_shard)
     double *Ksr = nullptr, *Klr = nullptr, *Astack = nullptr, *Zstack = nullptr, *rho = nullptr;
     double *hostP = nullptr, *hostJ = nullptr, *hostK = nullptr;     // device staging of build_host
+    double *noalloc_scratch = nullptr;   // device address of the static scratch of pbc_jk_overlap_noalloc (resolved at create)
+    cudaError_t noalloc_err = cudaSuccess;
     double *LT = nullptr, *chol_d = nullptr, *chol_s = nullptr;      // factor P' = L L^T of the K^LR contraction
     int *chol_dyn = nullptr;
     unsigned long long *maxbits = nullptr, *counters = nullptr;
@@ -806,6 +808,10 @@ int pbc_jk_create(const pbc_cell *cell, const pbc_atoms *atoms, const pbc_shells
         delete h;
         return fail(nullptr, PBC_JK_ERR_CUDA, "cannot query the current CUDA device");
     }
+    // set-up of pbc_jk_overlap_noalloc: the device address of its file-scope scratch array (once per device, this device
+    // current); a failure is reported by that entry point, not here
+    h->noalloc_err = noalloc_scratch_address(h->device, &h->noalloc_scratch);
+    if (h->noalloc_err != cudaSuccess) cudaGetLastError();
     const auto t0 = std::chrono::steady_clock::now();
     int rc;
     try {
@@ -833,6 +839,33 @@ int pbc_jk_overlap(const pbc_jk *h, double *S_host)
 {
     if (!h || !S_host) return PBC_JK_ERR_INVALID_ARG;
     std::memcpy(S_host, h->S_host.data(), h->S_host.size() * sizeof(double));
+    return PBC_JK_OK;
+}
+
+static_assert(NOALLOC_MAX_NP == PBC_JK_NOALLOC_MAX_NBF, "header and kernel file disagree on the static scratch size");
+
+int pbc_jk_overlap_noalloc(pbc_jk *h, double *S_dev, void *cuda_stream)
+{
+    if (!h) return PBC_JK_ERR_INVALID_ARG;
+    if (!S_dev) return fail(h, PBC_JK_ERR_INVALID_ARG, "S_dev is null");
+    if (h->Np > NOALLOC_MAX_NP) {
+        char buf[200];
+        std::snprintf(buf, sizeof buf, "pbc_jk_overlap_noalloc: N = %d (padded to %d) exceeds the static scratch, sized for at most %d "
+                      "basis functions", h->N, h->Np, NOALLOC_MAX_NP);
+        return fail(h, PBC_JK_ERR_UNSUPPORTED, buf);
+    }
+    {
+        int dev = -1;
+        CK(cudaGetDevice(&dev));
+        if (dev != h->device) return fail(h, PBC_JK_ERR_INVALID_ARG, "the handle was created on another CUDA device than the current one");
+    }
+    if (h->noalloc_err != cudaSuccess || !h->noalloc_scratch) {
+        char buf[200];
+        std::snprintf(buf, sizeof buf, "pbc_jk_overlap_noalloc: cudaGetSymbolAddress of the static scratch failed at create: %s",
+                      cudaGetErrorString(h->noalloc_err));
+        return fail(h, PBC_JK_ERR_CUDA, buf);
+    }
+    CK(launch_overlap_noalloc(h->lr, h->noalloc_scratch, h->N, S_dev, (cudaStream_t)cuda_stream));
     return PBC_JK_OK;
 }
 

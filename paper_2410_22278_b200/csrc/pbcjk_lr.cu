@@ -12,6 +12,7 @@
 #include "pbcjk_md.cuh"
 #include <algorithm>
 #include <cmath>
+#include <mutex>
 
 namespace pbcjk {
 
@@ -869,6 +870,46 @@ void launch_extract_overlap(const double *Astack, int Np, int S, int N, const do
 {
     dim3 grid((N + 127) / 128, N);
     extract_overlap_kernel<<<grid, 128, 0, st>>>(Astack, (size_t)Np * S, S, N, fcomp, Sm);
+}
+
+// ---------------------------------------------------------------- allocation-free overlap (pbc_jk_overlap_noalloc)
+// The crystalline overlap S = rho_mn(G = 0) (eq 21) is formed by agen_kernel in a scratch stack A'[m][n][slot] and read out
+// by extract_overlap_kernel.  This variant keeps that scratch (2 slots per element) in a file-scope device array, so the
+// call allocates nothing.  Every GPU that loads the library holds the array (NOALLOC_MAX_NP^2 * 2 doubles = 4 MiB) until
+// the process exits; all calls share it (calls that overlap on the GPU race) and it keeps the last call's contents, so
+// every call clears the part it reads (elements of shell pairs without a primitive pair-image are never written by agen).
+constexpr int NOALLOC_SLOTS = 2;                          // (Re, Im) of the one "G vector" of the overlap mode
+static __device__ __align__(256) double g_noalloc_scratch[(size_t)NOALLOC_MAX_NP * NOALLOC_MAX_NP * NOALLOC_SLOTS];
+
+// Set-up, once per device, with that device current: in host code `g_noalloc_scratch` is a host-side stand-in, not a device
+// address -- the address the kernels need comes from cudaGetSymbolAddress.
+cudaError_t noalloc_scratch_address(int device, double **ptr)
+{
+    static std::mutex mtx;
+    static double *cache[64] = {};
+    *ptr = nullptr;
+    if (device < 0 || device >= 64) return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lock(mtx);
+    if (!cache[device]) {
+        void *a = nullptr;
+        const cudaError_t e = cudaGetSymbolAddress(&a, g_noalloc_scratch);
+        if (e != cudaSuccess) return e;
+        cache[device] = static_cast<double *>(a);
+    }
+    *ptr = cache[device];
+    return cudaSuccess;
+}
+
+// scratch: the device address from noalloc_scratch_address; S_out: N x N, device.  Enqueues a clear, the agen kernels and the
+// read-out on `st`; no allocation, no synchronisation.
+cudaError_t launch_overlap_noalloc(const LRParams &p, double *scratch, int N, double *S_out, cudaStream_t st)
+{
+    if (p.Np > NOALLOC_MAX_NP) return cudaErrorInvalidValue;
+    const cudaError_t e = cudaMemsetAsync(scratch, 0, (size_t)p.Np * p.Np * NOALLOC_SLOTS * sizeof(double), st);
+    if (e != cudaSuccess) return e;
+    launch_agen(p, -1, 1, NOALLOC_SLOTS, 1.0, scratch, nullptr, nullptr, st);
+    launch_extract_overlap(scratch, p.Np, NOALLOC_SLOTS, N, p.fcomp, S_out, st);
+    return cudaGetLastError();
 }
 
 }  // namespace pbcjk

@@ -79,5 +79,11 @@ void launch_finalize_j(const double *Jsr, const double *Jlr, int N, const double
 void launch_finalize_k(const double *Ksr, const ShellInfo &sh, const double *Klr, int nsplit, size_t strideK, int Np,
                        int N, const double *fcomp, const int *shell_of_ao, double *K, cudaStream_t st);
 void launch_extract_overlap(const double *Astack, int Np, int S, int N, const double *fcomp, double *Sm, cudaStream_t st);
+// allocation-free overlap (pbc_jk_overlap_noalloc): the scratch stack lives in a file-scope device array of pbcjk_lr.cu
+// (NOALLOC_MAX_NP^2 * 2 doubles = 4 MiB); noalloc_scratch_address resolves its device address once per device (device current),
+// launch_overlap_noalloc clears what it needs, runs the agen kernels into it and reads S out -- no allocation.
+constexpr int NOALLOC_MAX_NP = 512;       // largest padded basis size N_p (multiple of 64) the static scratch holds
+cudaError_t noalloc_scratch_address(int device, double **ptr);
+cudaError_t launch_overlap_noalloc(const LRParams &p, double *scratch, int N, double *S_out, cudaStream_t st);
 
 }  // namespace pbcjk
