@@ -155,6 +155,12 @@ def _ncu_traffic(kernel):
     return None
 
 
+def _pair_traffic():
+    """DRAM bytes of one dgemm_kernel<0,0> + dgemm_kernel<0,1> launch pair (the unit of the GEMM roofline), or None"""
+    a, b = _ncu_traffic("dgemm_kernel<0,0>"), _ncu_traffic("dgemm_kernel<0,1>")
+    return a + b if a is not None and b is not None else None
+
+
 def h_nb(st, n):
     """G vectors per reciprocal-space batch as pbc_jk_create sizes them (stacks <= 12 GB, at most 64)"""
     np_ = ((n + 63) // 64) * 64
@@ -449,7 +455,7 @@ def main():
                                           "gemm_inner_loop_no_global_loads": round(pk["fp64_dmma_loop"], 2)},
                    "flop_per_launch_pair": gemm_flop / max(1, n_gemm_launch // 2), "rank_of_P": r_p, "g_slots": slots,
                    "ms_per_launch_pair": gemm_ms / max(1, n_gemm_launch // 2),
-                   "traffic": _ncu_traffic("dgemm_kernel<0,0>"),
+                   "traffic": _pair_traffic(),
                    "ms_lr_phase": st["ms_lr"]}
         top, other = (lr_gemm, real_space) if gemm_ms >= sr_ms else (real_space, lr_gemm)
         roofline = dict(top)
