@@ -455,7 +455,7 @@ def main():
                                           "gemm_inner_loop_no_global_loads": round(pk["fp64_dmma_loop"], 2)},
                    "flop_per_launch_pair": gemm_flop / max(1, n_gemm_launch // 2), "rank_of_P": r_p, "g_slots": slots,
                    "ms_per_launch_pair": gemm_ms / max(1, n_gemm_launch // 2),
-                   "traffic": _pair_traffic(),
+                   "traffic": _pair_traffic() if args.workload == "water64" and world == 1 else None,   # the capture is water64's
                    "ms_lr_phase": st["ms_lr"]}
         top, other = (lr_gemm, real_space) if gemm_ms >= sr_ms else (real_space, lr_gemm)
         roofline = dict(top)
