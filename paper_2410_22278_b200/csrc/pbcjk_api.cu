@@ -619,6 +619,8 @@ int setup(pbc_jk *h, const pbc_cell *cell, const pbc_atoms *atoms, const pbc_she
         }
         for (int g = 0; g < natom * 5; ++g) off[g + 1] += off[g];
         KetListJ &KJ = h->KJ;
+        if (n >= ((size_t)1 << J_KET_BITS))
+            return fail(h, PBC_JK_ERR_UNSUPPORTED, "more than 2^26 primitive pair-images in the J-engine ket list (packed ring entries)");
         KJ.n = (int)n; KJ.ngroup = natom; KJ.dstride = (int64_t)std::max<size_t>(n, 1);
         CK(pool.upload(&KJ.Qx, Qx)); CK(pool.upload(&KJ.Qy, Qy)); CK(pool.upload(&KJ.Qz, Qz));
         CK(pool.upload(&KJ.q, q)); CK(pool.upload(&KJ.iq, iq)); CK(pool.upload(&KJ.coef, coef)); CK(pool.upload(&KJ.lb, lb));

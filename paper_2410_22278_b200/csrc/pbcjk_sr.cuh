@@ -20,6 +20,7 @@
 // The fp32 screen keeps a superset of the fp64 rule (slack SCREEN_MARGIN in the logarithm of the bound).
 #pragma once
 #include "pbcjk_md.cuh"
+#include <type_traits>
 
 namespace pbcjk {
 
@@ -48,7 +49,12 @@ struct SRParams {
     unsigned long long *counters;
 };
 
-constexpr int QCAP = 64;        // survivor ring per warp (power of two)
+#ifndef J_UNR
+#define J_UNR 6                 // candidate passes per screening step
+#endif
+constexpr int J_KET_BITS = 26;  // ring entries pack (ket, image): at most 2^26 J kets (checked at create), NIMG_J = 64 images per chunk
+constexpr int QCAP = 256;       // survivor ring per warp (power of two): up to 31 queued + 32 * J_UNR new survivors per screening step
+static_assert(31 + 32 * J_UNR <= QCAP, "ring too small");
 constexpr int NIMG_J = 64;      // lattice images per warp-level list chunk (J-engine)
 
 __device__ __forceinline__ void lattice_T(const Lattice &lat, int n0, int n1, int n2, double &Tx, double &Ty, double &Tz)
@@ -108,7 +114,7 @@ __global__ void __launch_bounds__(128) sr_j_kernel(SRParams p, const int *__rest
 {
     constexpr int L = LB + LK;
     constexpr int NT = nherm(LB), NS = nherm(LK);
-    __shared__ int2 s_queue[4][QCAP];
+    __shared__ unsigned s_queue[4][QCAP];                       // ket index | image index << J_KET_BITS
     __shared__ double s_T[4][3][NIMG_J];
     __shared__ float s_C[4][3][NIMG_J];
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
@@ -131,7 +137,7 @@ __global__ void __launch_bounds__(128) sr_j_kernel(SRParams p, const int *__rest
     double Jt[NT];
 #pragma unroll
     for (int t = 0; t < NT; ++t) Jt[t] = 0.0;
-    int2 *queue = s_queue[w];
+    unsigned *queue = s_queue[w];
     double *sT = &s_T[w][0][0];
     float *sC = &s_C[w][0][0];
     const unsigned ltmask = (1u << lane) - 1u;
@@ -225,31 +231,50 @@ __global__ void __launch_bounds__(128) sr_j_kernel(SRParams p, const int *__rest
                     have = true;
                 }
                 if (jpos >= c_cnt) { have = false; continue; }
-                const int jj = jpos + lane;
-                jpos += 32;
-                bool pass = false;
-                if (jj < c_cnt) {
-                    const int j = c_k0 + jj;
-                    const float4 k4 = __ldg(KJ.q4 + j);                           // (Q - atom).xyz, lb
-                    const float iq = __ldg(KJ.iqf + j);
-                    const float ex = k4.x - c_Dx, ey = k4.y - c_Dy, ez = k4.z - c_Dz;   // Q + T - P
-                    const float r2 = ex * ex + ey * ey + ez * ez;
-                    const float isum = ipi + iq + iw2;
-                    pass = (thr + k4.w + M) * isum > r2 && r2 <= rcut2f;
-                    if (pass) pass = (thrx + k4.w + __ldg(p.kjP + j) + M) * isum > r2;   // per-block max |P'| (L819)
-                    ++ncand;
-                }
-                const unsigned m = __ballot_sync(0xffffffffu, pass);
-                if (pass) queue[(head + qn + __popc(m & ltmask)) & (QCAP - 1)] = make_int2(c_k0 + jj, c_t);
-                qn += __popc(m);
+                // Several passes of 32 candidates per step -- 2, or J_UNR when the item still holds more than 64 --: all
+                // records are requested before any is tested (a pass is a chain of dependent loads and a ballot: the scan is
+                // bound by that latency, not by issue slots; si64 J 625 -> 492 ms, water64 120 -> 116 ms)
+                auto passes = [&](auto UC) {
+                    constexpr int U = decltype(UC)::value;
+                    const int jbase = jpos + lane;
+                    const int npass = min(U, (c_cnt - jpos + 31) >> 5);        // warp-uniform
+                    jpos += 32 * U;
+                    float4 k4[U];
+                    float iq[U], kp[U];
+#pragma unroll
+                    for (int u2 = 0; u2 < U; ++u2) {
+                        const int jj = jbase + 32 * u2;
+                        k4[u2] = make_float4(0.f, 0.f, 0.f, 0.f); iq[u2] = 0.f; kp[u2] = 0.f;
+                        if (jj < c_cnt) { k4[u2] = __ldg(KJ.q4 + c_k0 + jj); iq[u2] = __ldg(KJ.iqf + c_k0 + jj); kp[u2] = __ldg(p.kjP + c_k0 + jj); }
+                    }
+#pragma unroll
+                    for (int u2 = 0; u2 < U; ++u2) {
+                        if (u2 < npass) {
+                            const int jj = jbase + 32 * u2;
+                            bool pass = false;
+                            if (jj < c_cnt) {
+                                const float ex = k4[u2].x - c_Dx, ey = k4[u2].y - c_Dy, ez = k4[u2].z - c_Dz;   // Q + T - P
+                                const float r2 = ex * ex + ey * ey + ez * ez;
+                                const float isum = ipi + iq[u2] + iw2;
+                                pass = (thrx + k4[u2].w + kp[u2] + M) * isum > r2 && r2 <= rcut2f;   // per-block max |P'| (L819)
+                                ++ncand;
+                            }
+                            const unsigned m = __ballot_sync(0xffffffffu, pass);
+                            if (pass) queue[(head + qn + __popc(m & ltmask)) & (QCAP - 1)] = (unsigned)(c_k0 + jj) | ((unsigned)c_t << J_KET_BITS);
+                            qn += __popc(m);
+                        }
+                    }
+                };
+                if (c_cnt - jpos > 64) passes(std::integral_constant<int, J_UNR>());
+                else passes(std::integral_constant<int, 2>());
                 __syncwarp();
             }
             if (!(qn >= 32 || (items_done && qn > 0))) break;
             // ---- evaluation: one primitive quartet-image per lane ----
             const int take = qn < 32 ? qn : 32;
             if (lane < take) {
-                const int2 e = queue[(head + lane) & (QCAP - 1)];
-                const int j = e.x, t = e.y;
+                const unsigned e = queue[(head + lane) & (QCAP - 1)];
+                const int j = (int)(e & ((1u << J_KET_BITS) - 1u)), t = (int)(e >> J_KET_BITS);
                 const double X = __ldg(KJ.Qx + j) + sT[t] - Pix, Y = __ldg(KJ.Qy + j) + sT[NIMG_J + t] - Piy,
                              Z = __ldg(KJ.Qz + j) + sT[2 * NIMG_J + t] - Piz;
                 const double q = __ldg(KJ.q + j);
