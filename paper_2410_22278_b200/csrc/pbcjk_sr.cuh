@@ -183,6 +183,7 @@ __global__ void __launch_bounds__(128) sr_j_kernel(SRParams p, const int *__rest
         }
         __syncwarp();
         const int nitems = natom * nimg;
+        const float inv_nimg = 1.f / (float)max(nimg, 1);
         int ebase = 0;
         unsigned imask = 0;
         bool have = false, items_done = false;
@@ -200,7 +201,8 @@ __global__ void __launch_bounds__(128) sr_j_kernel(SRParams p, const int *__rest
                         ebase += 32;
                         it_cnt = 0;
                         if (e < nitems) {
-                            const int a = e / nimg, t = e - a * nimg;
+                            int a = (int)((float)e * inv_nimg), t = e - a * nimg;       // e / nimg without the integer division
+                            if (t < 0) { --a; t += nimg; } else if (t >= nimg) { ++a; t -= nimg; }
                             const int gi = a * 5 + LK;
                             const int2 go = __ldg(KJ.goff + gi);                   // (first ket, count)
                             if (go.y > 0) {

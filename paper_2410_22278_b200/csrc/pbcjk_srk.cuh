@@ -183,6 +183,7 @@ sr_k_kernel(SRParams p, const int2 *__restrict__ blocks, int nblocks)
         const int nimg = s_ctl[0];
         ibox = s_ctl[1];
         const int nitems = nb_eff * nimg;
+        const float inv_nimg = 1.f / (float)max(nimg, 1);
         int ebase = w * 32;
         unsigned imask = 0;
         bool have = false, items_done = false;
@@ -200,7 +201,8 @@ sr_k_kernel(SRParams p, const int2 *__restrict__ blocks, int nblocks)
                         ebase += 32 * NW;
                         it_cnt = 0;
                         if (e < nitems) {
-                            const int ib = e / nimg, t = e - ib * nimg;
+                            int ib = (int)((float)e * inv_nimg), t = e - ib * nimg;   // e / nimg without the integer division
+                            if (t < 0) { --ib; t += nimg; } else if (t >= nimg) { ++ib; t -= nimg; }
                             const int i = b0 + ib;
                             const float4 b4 = __ldg(K.q4 + i);                     // (P - mu).xyz, lb
                             const float ipi = __ldg(K.ipf + i);
