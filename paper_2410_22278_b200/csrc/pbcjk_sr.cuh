@@ -91,15 +91,25 @@ struct ImageBox {
     }
 };
 
-// number of leading entries of a list sorted by descending bound (q4[].w) that exceed `need` (per lane)
+// number of leading entries of a list sorted by descending bound (q4[].w) that exceed `need` (per lane).
+// Four-way search: the three pivots of a step are independent loads, so the chain of dependent loads is half as long as that
+// of a binary search (level A of the screens waits on this chain in nearly every batch of 32 items).
 __device__ __forceinline__ int count_above_sorted(const float4 *__restrict__ q4, int n, float need)
 {
-    int lo = 0, hi = n;
-    while (lo < hi) {
-        const int mid = (lo + hi) >> 1;
-        if (__ldg(&q4[mid].w) > need) lo = mid + 1;
-        else hi = mid;
+    int lo = 0, hi = n;                                      // invariant: entries < lo exceed need, entries >= hi do not
+    while (hi - lo > 3) {
+        const int q = (hi - lo) >> 2;
+        const int m1 = lo + q, m2 = lo + 2 * q, m3 = lo + 3 * q;
+        const float v1 = __ldg(&q4[m1].w), v2 = __ldg(&q4[m2].w), v3 = __ldg(&q4[m3].w);
+        if (v2 > need) {
+            if (v3 > need) lo = m3 + 1;
+            else { lo = m2 + 1; hi = m3; }
+        } else {
+            if (v1 > need) { lo = m1 + 1; hi = m2; }
+            else hi = m1;
+        }
     }
+    while (lo < hi && __ldg(&q4[lo].w) > need) ++lo;         // at most three entries left
     return lo;
 }
 
