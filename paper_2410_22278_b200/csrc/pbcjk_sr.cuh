@@ -277,7 +277,43 @@ __global__ void __launch_bounds__(128) sr_j_kernel(SRParams p, const int *__rest
                         }
                     }
                 };
-                if (c_cnt - jpos > 64) passes(std::integral_constant<int, J_UNR>());
+                if (c_cnt - jpos <= 32 && imask != 0) {
+                    // the last pass of this item runs together with the first pass of the next live item of the batch (an
+                    // item holds 12 candidates on average on water64: one item per step is one latency chain per item)
+                    const int src = __ffs(imask) - 1;
+                    imask &= imask - 1;
+                    const int d_cnt = __shfl_sync(0xffffffffu, it_cnt, src), d_k0 = __shfl_sync(0xffffffffu, it_k0, src),
+                              d_t = __shfl_sync(0xffffffffu, it_t, src);
+                    const float d_Dx = __shfl_sync(0xffffffffu, it_Dx, src), d_Dy = __shfl_sync(0xffffffffu, it_Dy, src),
+                                d_Dz = __shfl_sync(0xffffffffu, it_Dz, src);
+                    const int jj0 = jpos + lane, jj1 = lane;
+                    const bool va = jj0 < c_cnt, vb = jj1 < d_cnt;
+                    float4 ka = make_float4(0.f, 0.f, 0.f, 0.f), kb = ka;
+                    float iqa = 0.f, iqb = 0.f, kpa = 0.f, kpb = 0.f;
+                    if (va) { ka = __ldg(KJ.q4 + c_k0 + jj0); iqa = __ldg(KJ.iqf + c_k0 + jj0); kpa = __ldg(p.kjP + c_k0 + jj0); }
+                    if (vb) { kb = __ldg(KJ.q4 + d_k0 + jj1); iqb = __ldg(KJ.iqf + d_k0 + jj1); kpb = __ldg(p.kjP + d_k0 + jj1); }
+                    bool pa = false, pb = false;
+                    if (va) {
+                        const float ex = ka.x - c_Dx, ey = ka.y - c_Dy, ez = ka.z - c_Dz;
+                        const float r2 = ex * ex + ey * ey + ez * ez;
+                        pa = (thrx + ka.w + kpa + M) * (ipi + iqa + iw2) > r2 && r2 <= rcut2f;
+                        ++ncand;
+                    }
+                    if (vb) {
+                        const float ex = kb.x - d_Dx, ey = kb.y - d_Dy, ez = kb.z - d_Dz;
+                        const float r2 = ex * ex + ey * ey + ez * ez;
+                        pb = (thrx + kb.w + kpb + M) * (ipi + iqb + iw2) > r2 && r2 <= rcut2f;
+                        ++ncand;
+                    }
+                    const unsigned ma = __ballot_sync(0xffffffffu, pa);
+                    if (pa) queue[(head + qn + __popc(ma & ltmask)) & (QCAP - 1)] = (unsigned)(c_k0 + jj0) | ((unsigned)c_t << J_KET_BITS);
+                    qn += __popc(ma);
+                    const unsigned mb = __ballot_sync(0xffffffffu, pb);
+                    if (pb) queue[(head + qn + __popc(mb & ltmask)) & (QCAP - 1)] = (unsigned)(d_k0 + jj1) | ((unsigned)d_t << J_KET_BITS);
+                    qn += __popc(mb);
+                    c_cnt = d_cnt; c_k0 = d_k0; c_t = d_t; c_Dx = d_Dx; c_Dy = d_Dy; c_Dz = d_Dz;
+                    jpos = 32;
+                } else if (c_cnt - jpos > 64) passes(std::integral_constant<int, J_UNR>());
                 else passes(std::integral_constant<int, 2>());
                 __syncwarp();
             }
