@@ -54,6 +54,9 @@ constexpr int KQ = 64;                                       // ring capacity pe
 __host__ __device__ constexpr bool k_lockstep(int L, bool mixed) { return L >= K_LOCK_LMIN && !mixed; }
 __host__ __device__ constexpr int k_ring(int L, bool mixed) { return k_lockstep(L, mixed) ? 128 : KQ; }
 __host__ __device__ constexpr int k_qstop(int L, bool mixed) { return k_lockstep(L, mixed) ? 64 : 32; }
+#ifndef K_PAIR
+#define K_PAIR 1                                              // level B: pair an item's last pass with the next item's first
+#endif
 constexpr int NIMG_K = 128;                                  // lattice images per CTA-level list chunk
 
 
@@ -233,36 +236,62 @@ sr_k_kernel(SRParams p, const int2 *__restrict__ blocks, int nblocks)
                     have = true;
                 }
                 if (jpos >= c_cnt) { have = false; continue; }
-                const int jj = jpos + lane;
-                jpos += 32;
-                bool pass = false, lo32 = false;
-                if (jj < c_cnt) {
-                    const float4 k4 = __ldg(kq4 + jj);                            // (Q - nu).xyz, lb
-                    const float iq = __ldg(kipf + jj);
-                    const float ex = k4.x - c_Dx, ey = k4.y - c_Dy, ez = k4.z - c_Dz;   // Q + T - P
-                    const float r2 = ex * ex + ey * ey + ez * ez;
-                    const float isum = c_ipi + iq + iw2;
-                    pass = (c_thr + k4.w + M) * isum > r2 && r2 <= rcut2f;
-                    ++ncand;
-                    if (pass) {                                                   // max |P'| over the shell block (L819)
-                        const int i = b0 + (c_ibt & 0xffff);
-                        const float lbsum = __ldg(&K.q4[i].w) + k4.w +
-                                            __ldg(p.lnPblk + (size_t)__ldg(K.shB + i) * ns + __ldg(kshB + jj));
-                        pass = (lbsum - ln_tau + M) * isum > r2;
-                        if constexpr (MIXED)
-                            lo32 = pass && lbsum < p.ln_switch && __ldg(K.rng + i) + __ldg(K.rng + k0 + jj) < 60.f;
+                // test of one candidate per lane (screen record k4, 1/q already loaded) and compaction of the survivors
+                auto test_push = [&](int jj, bool valid, const float4 &k4, float iq, int ibt, float Dx, float Dy, float Dz, float thr, float ipi) {
+                    bool pass = false, lo32 = false;
+                    if (valid) {
+                        const float ex = k4.x - Dx, ey = k4.y - Dy, ez = k4.z - Dz;   // Q + T - P
+                        const float r2 = ex * ex + ey * ey + ez * ez;
+                        const float isum = ipi + iq + iw2;
+                        pass = (thr + k4.w + M) * isum > r2 && r2 <= rcut2f;
+                        ++ncand;
+                        if (pass) {                                               // max |P'| over the shell block (L819)
+                            const int i = b0 + (ibt & 0xffff);
+                            const float lbsum = __ldg(&K.q4[i].w) + k4.w +
+                                                __ldg(p.lnPblk + (size_t)__ldg(K.shB + i) * ns + __ldg(kshB + jj));
+                            pass = (lbsum - ln_tau + M) * isum > r2;
+                            if constexpr (MIXED)
+                                lo32 = pass && lbsum < p.ln_switch && __ldg(K.rng + i) + __ldg(K.rng + k0 + jj) < 60.f;
+                        }
                     }
-                }
-                if constexpr (MIXED) {
-                    const unsigned m32 = __ballot_sync(0xffffffffu, lo32), m64 = __ballot_sync(0xffffffffu, pass && !lo32);
-                    if (lo32) queue32[(head32 + qn32 + __popc(m32 & ltmask)) & (KQ - 1)] = make_int2((c_ibt & 0xffff) | (jj << 16), c_ibt >> 16);
-                    else if (pass) queue[(head + qn + __popc(m64 & ltmask)) & (KQ - 1)] = make_int2((c_ibt & 0xffff) | (jj << 16), c_ibt >> 16);
-                    qn32 += __popc(m32);
-                    qn += __popc(m64);
+                    if constexpr (MIXED) {
+                        const unsigned m32 = __ballot_sync(0xffffffffu, lo32), m64 = __ballot_sync(0xffffffffu, pass && !lo32);
+                        if (lo32) queue32[(head32 + qn32 + __popc(m32 & ltmask)) & (KQ - 1)] = make_int2((ibt & 0xffff) | (jj << 16), ibt >> 16);
+                        else if (pass) queue[(head + qn + __popc(m64 & ltmask)) & (KQ - 1)] = make_int2((ibt & 0xffff) | (jj << 16), ibt >> 16);
+                        qn32 += __popc(m32);
+                        qn += __popc(m64);
+                    } else {
+                        const unsigned m = __ballot_sync(0xffffffffu, pass);
+                        if (pass) queue[(head + qn + __popc(m & ltmask)) & (KQ - 1)] = make_int2((ibt & 0xffff) | (jj << 16), ibt >> 16);
+                        qn += __popc(m);
+                    }
+                };
+                const int jj = jpos + lane;
+                const bool va = jj < c_cnt;
+                float4 ka = make_float4(0.f, 0.f, 0.f, 0.f);
+                float iqa = 0.f;
+                if (va) { ka = __ldg(kq4 + jj); iqa = __ldg(kipf + jj); }          // (Q - nu).xyz, lb; 1/q
+                if (K_PAIR && !MIXED && c_cnt - jpos <= 32 && imask != 0 && qn + (c_cnt - jpos) + 32 <= KQ) {   // (the ring takes both passes)
+                    // the last pass of this item runs together with the first pass of the next live item of the batch (both
+                    // records are requested before either is tested: a pass is a chain of dependent loads and a ballot); water64 K
+                    // 365 -> 359 ms, water343 3038 -> 3004 ms; the mixed-precision kernels (two rings) lose 1 % with it
+                    const int src = __ffs(imask) - 1;
+                    imask &= imask - 1;
+                    const int d_ibt = __shfl_sync(0xffffffffu, it_ibt, src), d_cnt = __shfl_sync(0xffffffffu, it_cnt, src);
+                    const float d_Dx = __shfl_sync(0xffffffffu, it_Dx, src), d_Dy = __shfl_sync(0xffffffffu, it_Dy, src),
+                                d_Dz = __shfl_sync(0xffffffffu, it_Dz, src), d_thr = __shfl_sync(0xffffffffu, it_thr, src),
+                                d_ipi = __shfl_sync(0xffffffffu, it_ipi, src);
+                    const bool vb = lane < d_cnt;
+                    float4 kb = make_float4(0.f, 0.f, 0.f, 0.f);
+                    float iqb = 0.f;
+                    if (vb) { kb = __ldg(kq4 + lane); iqb = __ldg(kipf + lane); }
+                    test_push(jj, va, ka, iqa, c_ibt, c_Dx, c_Dy, c_Dz, c_thr, c_ipi);
+                    test_push(lane, vb, kb, iqb, d_ibt, d_Dx, d_Dy, d_Dz, d_thr, d_ipi);
+                    c_ibt = d_ibt; c_cnt = d_cnt; c_Dx = d_Dx; c_Dy = d_Dy; c_Dz = d_Dz; c_thr = d_thr; c_ipi = d_ipi;
+                    jpos = 32;
                 } else {
-                    const unsigned m = __ballot_sync(0xffffffffu, pass);
-                    if (pass) queue[(head + qn + __popc(m & ltmask)) & (KQ - 1)] = make_int2((c_ibt & 0xffff) | (jj << 16), c_ibt >> 16);
-                    qn += __popc(m);
+                    jpos += 32;
+                    test_push(jj, va, ka, iqa, c_ibt, c_Dx, c_Dy, c_Dz, c_thr, c_ipi);
                 }
                 __syncwarp();
             }
